@@ -1,0 +1,819 @@
+// api.cu -- host side of liberi_b200: the C ABI of include/eri.h, the plan builder (shell grouping, pair sets,
+// Schwarz bounds, Schwarz-sorted task lists; Algorithm 1 lines 1-8) and kernel dispatch.
+// Product code: there is no CPU fallback and nothing from oracle/ is used here.
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/eri.h"
+#include "eri_dev.cuh"
+#include "launch.h"
+#include "rys_tables.inc"
+
+namespace eri {
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+  g_err = buf;
+  return code;
+}
+#define CK(call)                                                                                       \
+  do {                                                                                                 \
+    cudaError_t e_ = (call);                                                                           \
+    if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? ERI_ERR_NOMEM : ERI_ERR_CUDA, \
+                                       "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+  } while (0)
+#define CKI(call) do { int r_ = (call); if (r_ != ERI_OK) return r_; } while (0)
+
+template <class T>
+struct Dev {   // owning device array
+  T* p = nullptr; size_t n = 0;
+  Dev() = default;
+  Dev(const Dev&) = delete; Dev& operator=(const Dev&) = delete;
+  Dev(Dev&& o) noexcept : p(o.p), n(o.n) { o.p = nullptr; o.n = 0; }
+  Dev& operator=(Dev&& o) noexcept { if (this != &o) { release(); p = o.p; n = o.n; o.p = nullptr; o.n = 0; } return *this; }
+  ~Dev() { release(); }
+  void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+  cudaError_t alloc(size_t count) {
+    release();
+    if (count == 0) return cudaSuccess;
+    n = count;
+    return cudaMalloc(&p, count * sizeof(T));
+  }
+  cudaError_t upload(const std::vector<T>& h, cudaStream_t s) {
+    cudaError_t e = alloc(h.size());
+    if (e != cudaSuccess || h.empty()) return e;
+    return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+  }
+};
+
+// ---- process-wide read-only device data ---------------------------------------------------------------------
+std::mutex g_init_mu;
+double* g_rys = nullptr;
+bool g_c2s_ready = false;
+std::vector<double> g_c2s_host[LMAX + 1];
+
+double binom(int n, int k) { if (k < 0 || k > n) return 0.0; double r = 1.0; for (int i = 1; i <= k; ++i) r = r * (n - k + i) / i; return r; }
+double fact(int n) { double r = 1.0; for (int i = 2; i <= n; ++i) r *= i; return r; }
+int cart_index(int l, int lx, int ly) {  // lx descending, then ly descending
+  int idx = 0;
+  for (int x = l; x > lx; --x) idx += l - x + 1;
+  return idx + (l - lx - ly);
+}
+
+// Real solid harmonics, unit-normalised on the sphere, m = -l..l (reading R3): closed formula
+//   Y_lm = sqrt((2l+1)/4pi) N_lm sum_{t,u,v} C^{lm}_{tuv} x^{2t+|m|-2(u+v)} y^{2(u+v)} z^{l-2t-|m|}.
+void build_c2s(int l, std::vector<double>& T) {
+  const int nc = ncart(l), ns = nsph(l);
+  T.assign((size_t)ns * nc, 0.0);
+  for (int m = -l; m <= l; ++m) {
+    const int am = std::abs(m);
+    const double Nlm = std::sqrt(2.0 * fact(l + am) * fact(l - am) / (m == 0 ? 2.0 : 1.0)) / (std::pow(2.0, am) * fact(l));
+    const double norm = std::sqrt((2 * l + 1) / (4.0 * PI)) * Nlm;
+    const int v2min = m < 0 ? 1 : 0;   // 2v runs over v2min, v2min+2, ... <= |m|
+    for (int t = 0; t <= (l - am) / 2; ++t)
+      for (int u = 0; u <= t; ++u)
+        for (int v2 = v2min; v2 <= am; v2 += 2) {
+          const int sign_exp = t + (v2 - v2min) / 2;
+          const double C = ((sign_exp & 1) ? -1.0 : 1.0) * std::pow(0.25, t) * binom(l, t) * binom(l - t, am + t) * binom(t, u) * binom(am, v2);
+          const int ex = 2 * t + am - (2 * u + v2), ey = 2 * u + v2, ez = l - 2 * t - am;
+          if (ex < 0 || ey < 0 || ez < 0) continue;
+          T[(size_t)(m + l) * nc + cart_index(l, ex, ey)] += norm * C;
+        }
+  }
+}
+
+int ensure_init() {
+  std::lock_guard<std::mutex> lk(g_init_mu);
+  if (!g_rys) {
+    // consistency of the compile-time constants in eri_dev.cuh with the generated table
+    for (int N = 1; N <= RYS_NMAX; ++N)
+      if (rys_offset(N) != RYS_TABLE_OFFSET_H[N] || rys_xmax(N) != RYS_XMAX_H[N])
+        return fail(ERI_ERR_BAD_ARG, "rys_tables.inc does not match eri_dev.cuh (N=%d)", N);
+    std::vector<double> h(RYS_HDR_SIZE + RYS_TABLE_SIZE, 0.0);
+    for (int N = 1; N <= RYS_NMAX; ++N) { h[RYS_HDR_XMAX + N] = RYS_XMAX_H[N]; h[RYS_HDR_OFF + N] = RYS_TABLE_OFFSET_H[N]; }
+    for (int k = 0; k < RYS_NMAX * (RYS_NMAX + 1) / 2; ++k) { h[RYS_HDR_H2 + k] = RYS_HERM_H2_H[k]; h[RYS_HDR_V + k] = RYS_HERM_V_H[k]; }
+    std::memcpy(h.data() + RYS_HDR_SIZE, RYS_TABLE_H, sizeof(double) * RYS_TABLE_SIZE);
+    double* d = nullptr;
+    CK(cudaMalloc(&d, h.size() * sizeof(double)));
+    CK(cudaMemcpy(d, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice));
+    g_rys = d;
+  }
+  if (!g_c2s_ready) {
+    std::vector<double> all;
+    for (int l = 0; l <= LMAX; ++l) { build_c2s(l, g_c2s_host[l]); all.insert(all.end(), g_c2s_host[l].begin(), g_c2s_host[l].end()); }
+    if (all.size() != 245) return fail(ERI_ERR_BAD_ARG, "internal: c2s table size");
+    CK(upload_c2s(all.data()));
+    g_c2s_ready = true;
+  }
+  return ERI_OK;
+}
+
+// ---- basis ----------------------------------------------------------------------------------------------------
+struct Group { int l, K; std::vector<int> shells; };
+
+struct Basis {
+  std::vector<eri_shell_t> sh; std::vector<eri_prim_t> pr; std::vector<double> xyz;
+  int natm = 0, nao = 0, nao_cart = 0;
+  std::vector<int> cart_off, group_of;
+  std::vector<Group> groups;   // sorted by (l, K)
+};
+
+int make_basis(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm, Basis& b) {
+  if (nshell < 0 || nprim < 0 || natm < 0) return fail(ERI_ERR_BAD_ARG, "negative count");
+  if ((nshell > 0 && (!shells || !prims || !coords))) return fail(ERI_ERR_BAD_ARG, "null basis pointer");
+  b.sh.assign(shells, shells + nshell); b.pr.assign(prims, prims + nprim); b.xyz.assign(coords, coords + 3 * (size_t)natm);
+  b.natm = natm; b.nao = 0; b.nao_cart = 0;
+  b.cart_off.resize(nshell); b.group_of.resize(nshell);
+  std::map<std::pair<int, int>, int> gid;
+  for (int s = 0; s < nshell; ++s) {
+    const eri_shell_t& S = shells[s];
+    if (S.l < 0 || S.l > LMAX) return fail(ERI_ERR_UNSUPPORTED_L, "shell %d: l = %d is outside 0..%d", s, S.l, LMAX);
+    if (S.nprim <= 0) return fail(ERI_ERR_BAD_ARG, "shell %d: nprim = %d", s, S.nprim);
+    if (S.prim_off < 0 || (long)S.prim_off + S.nprim > nprim) return fail(ERI_ERR_BAD_ARG, "shell %d: primitive range outside prims", s);
+    if (S.atom < 0 || S.atom >= natm) return fail(ERI_ERR_BAD_ARG, "shell %d: atom %d outside 0..%d", s, S.atom, natm - 1);
+    if (S.ao_off != b.nao) return fail(ERI_ERR_BAD_ARG, "shell %d: ao_off = %d, expected running sum %d", s, S.ao_off, b.nao);
+    for (int k = 0; k < S.nprim; ++k) {
+      const double e = prims[S.prim_off + k].exp, c = prims[S.prim_off + k].coef;
+      if (!(e > 0.0) || !std::isfinite(e) || !std::isfinite(c)) return fail(ERI_ERR_BAD_ARG, "shell %d: bad primitive %d", s, k);
+    }
+    b.cart_off[s] = b.nao_cart;
+    b.nao += nsph(S.l); b.nao_cart += ncart(S.l);
+    gid[{S.l, S.nprim}] = 0;
+  }
+  for (int x = 0; x < 3 * natm; ++x) if (!std::isfinite(coords[x])) return fail(ERI_ERR_BAD_ARG, "non-finite coordinate");
+  int g = 0;
+  for (auto& kv : gid) { kv.second = g++; b.groups.push_back(Group{kv.first.first, kv.first.second, {}}); }
+  for (int s = 0; s < nshell; ++s) { const int id = gid[{shells[s].l, shells[s].nprim}]; b.group_of[s] = id; b.groups[id].shells.push_back(s); }
+  return ERI_OK;
+}
+
+// ---- pair sets ------------------------------------------------------------------------------------------------
+struct PairClass {
+  int ga = 0, gb = 0, la = 0, lb = 0, Ka = 0, Kb = 0, npp = 0, npair = 0, stride = 0;
+  std::vector<int> sa, sb;       // shell ids, first / second
+  std::vector<double> Q, wgt;    // Schwarz factor, pair weight
+  Dev<double> prim, geom, aexp, q;
+  Dev<int2> ao, atom;
+  PairSet view() const {
+    PairSet v; v.prim = prim.p; v.geom = geom.p; v.aexp = aexp.p; v.q = q.p; v.ao = ao.p; v.atom = atom.p;
+    v.npair = npair; v.stride = stride; v.npp = npp; v.la = la; v.lb = lb; return v;
+  }
+};
+
+// fills and uploads the SoA arrays of pc from pc.sa/sb/wgt/Q (Q may be empty)
+int upload_pair_class(const Basis& b, PairClass& pc, cudaStream_t s) {
+  const int n = pc.npair = (int)pc.sa.size();
+  pc.stride = (n + 31) / 32 * 32;
+  if (n == 0) return ERI_OK;
+  const size_t st = pc.stride;
+  std::vector<double> prim((size_t)pc.npp * 5 * st, 0.0), geom(7 * st, 0.0), aexp((size_t)pc.npp * 2 * st, 0.0), q(st, 0.0);
+  std::vector<int2> ao(st, make_int2(0, 0)), atom(st, make_int2(0, 0));
+  const double kfac = std::sqrt(2.0) * std::pow(PI, 1.25);
+  for (int i = 0; i < n; ++i) {
+    const eri_shell_t& A = b.sh[pc.sa[i]]; const eri_shell_t& B = b.sh[pc.sb[i]];
+    const double* RA = &b.xyz[3 * A.atom]; const double* RB = &b.xyz[3 * B.atom];
+    const double ab[3] = {RA[0] - RB[0], RA[1] - RB[1], RA[2] - RB[2]};
+    const double r2 = ab[0] * ab[0] + ab[1] * ab[1] + ab[2] * ab[2];
+    for (int x = 0; x < 3; ++x) { geom[x * st + i] = RA[x]; geom[(3 + x) * st + i] = ab[x]; }
+    geom[6 * st + i] = pc.wgt.empty() ? 1.0 : pc.wgt[i];
+    ao[i] = make_int2(b.cart_off[pc.sa[i]], b.cart_off[pc.sb[i]]);
+    atom[i] = make_int2(A.atom, B.atom);
+    if (!pc.Q.empty()) q[i] = pc.Q[i];
+    int k = 0;
+    for (int ka = 0; ka < A.nprim; ++ka)
+      for (int kb = 0; kb < B.nprim; ++kb, ++k) {
+        const double ea = b.pr[A.prim_off + ka].exp, eb = b.pr[B.prim_off + kb].exp;
+        const double ca = b.pr[A.prim_off + ka].coef, cb = b.pr[B.prim_off + kb].coef;
+        const double p = ea + eb;
+        prim[((size_t)k * 5 + 0) * st + i] = p;
+        for (int x = 0; x < 3; ++x) prim[((size_t)k * 5 + 1 + x) * st + i] = (ea * RA[x] + eb * RB[x]) / p;
+        prim[((size_t)k * 5 + 4) * st + i] = kfac / p * ca * cb * std::exp(-ea * eb / p * r2);
+        aexp[((size_t)k * 2 + 0) * st + i] = ea; aexp[((size_t)k * 2 + 1) * st + i] = eb;
+      }
+  }
+  CK(pc.prim.upload(prim, s)); CK(pc.geom.upload(geom, s)); CK(pc.aexp.upload(aexp, s)); CK(pc.q.upload(q, s));
+  CK(pc.ao.upload(ao, s)); CK(pc.atom.upload(atom, s));
+  CK(cudaStreamSynchronize(s));   // the host vectors die here
+  return ERI_OK;
+}
+
+void init_pair_class(const Basis& b, int ga, int gb, PairClass& pc) {
+  pc.ga = ga; pc.gb = gb; pc.la = b.groups[ga].l; pc.lb = b.groups[gb].l; pc.Ka = b.groups[ga].K; pc.Kb = b.groups[gb].K;
+  pc.npp = pc.Ka * pc.Kb;
+}
+
+// Schwarz factors of every pair of pc (Eq. 7) through the generic store kernel on the quartets (ab|ab).
+int schwarz_of_class(PairClass& pc, cudaStream_t s) {
+  const int n = pc.npair;
+  pc.Q.assign(n, 0.0);
+  if (n == 0) return ERI_OK;
+  const long nab = (long)ncart(pc.la) * ncart(pc.lb), blk = nab * nab;
+  const int chunk = (int)std::max<long>(1, std::min<long>(n, (64L << 20) / blk));
+  Dev<double> cart, qd; Dev<int2> list; Dev<long long> off;
+  CK(cart.alloc((size_t)chunk * blk)); CK(qd.alloc(chunk));
+  std::vector<int2> hl(chunk); std::vector<long long> ho(chunk);
+  for (int start = 0; start < n; start += chunk) {
+    const int m = std::min(chunk, n - start);
+    for (int t = 0; t < m; ++t) { hl[t] = make_int2(start + t, start + t); ho[t] = (long long)t * blk; }
+    CK(list.upload(hl, s)); CK(off.upload(ho, s));
+    CK(cudaMemsetAsync(cart.p, 0, sizeof(double) * (size_t)m * blk, s));
+    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = list.p; w.nlist = m; w.rys = g_rys;
+    CK(launch_generic_store(w, cart.p, off.p, s));
+    CK(launch_schwarz_diag(pc.la, pc.lb, m, cart.p, qd.p, s));
+    CK(cudaMemcpyAsync(pc.Q.data() + start, qd.p, sizeof(double) * m, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+  }
+  return ERI_OK;
+}
+
+// ---- work units -----------------------------------------------------------------------------------------------
+struct Unit {
+  int P = 0, R = 0; bool same = false;
+  int BI = GENERIC_BI, BJ = GENERIC_BJ, nrows = 0, nblocks = 0;
+  int gBI = GENERIC_GRAD_BI, gBJ = GENERIC_GRAD_BJ, g_nrows = 0, g_nblocks = 0;
+  int kernel = 0, kernel_grad = 0;
+  long long quartets = 0;
+  double flops = 0, flops_grad = 0;
+  float last_ms = 0, last_ms_grad = 0;
+  std::vector<int> h_count;
+  Dev<int> ket_count, row_off, g_row_off;
+  Dev<int2> list; int nlist = 0;            // list mode
+  Dev<long long> coff;                      // list mode, store kernel
+};
+
+}  // namespace
+}  // namespace eri
+
+using namespace eri;
+
+struct eri_plan {
+  Basis basis;
+  bool is_list = false, want_grad = false;
+  double thr = 0.0;
+  int kernel_mode = 0, timing = 0;
+  std::vector<std::unique_ptr<PairClass>> pcs;
+  std::vector<std::unique_ptr<Unit>> units;
+  Dev<int> sh_l, sh_sph, sh_cart, sph2sh, cart2sh;
+  Dev<double> Dc, Jc, Kc, Dh, Jh, Kh, gJd, gKd;   // Cartesian workspaces; device staging for the *_host entry points
+  ShellMap map{};
+  eri_stats_t stats{};
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  ~eri_plan() { if (ev0) cudaEventDestroy(ev0); if (ev1) cudaEventDestroy(ev1); }
+};
+
+namespace eri {
+namespace {
+
+int make_shell_map(eri_plan& pl, cudaStream_t s) {
+  const Basis& b = pl.basis;
+  const int ns = (int)b.sh.size();
+  std::vector<int> l(ns), so(ns), co(ns), s2s(b.nao), c2s(b.nao_cart);
+  for (int i = 0; i < ns; ++i) {
+    l[i] = b.sh[i].l; so[i] = b.sh[i].ao_off; co[i] = b.cart_off[i];
+    for (int k = 0; k < nsph(l[i]); ++k) s2s[so[i] + k] = i;
+    for (int k = 0; k < ncart(l[i]); ++k) c2s[co[i] + k] = i;
+  }
+  CK(pl.sh_l.upload(l, s)); CK(pl.sh_sph.upload(so, s)); CK(pl.sh_cart.upload(co, s));
+  CK(pl.sph2sh.upload(s2s, s)); CK(pl.cart2sh.upload(c2s, s));
+  CK(cudaStreamSynchronize(s));
+  pl.map = ShellMap{pl.sh_l.p, pl.sh_sph.p, pl.sh_cart.p, pl.sph2sh.p, pl.cart2sh.p, ns, b.nao, b.nao_cart};
+  const size_t n2 = (size_t)b.nao_cart * b.nao_cart;
+  CK(pl.Dc.alloc(n2)); CK(pl.Jc.alloc(n2)); CK(pl.Kc.alloc(n2));
+  return ERI_OK;
+}
+
+double canonical_flops(int la, int lb, int lc, int ld, int ka, int kb, int kc, int kd, int deriv) {
+  // DESIGN.md "FLOP model" (FMA = 2): the work the Rys method has to do, independent of kernel organisation.
+  const int L = la + lb + lc + ld + (deriv ? 1 : 0), N = L / 2 + 1;
+  const int nmax = la + lb + (deriv ? 1 : 0), mmax = lc + ld + (deriv ? 1 : 0);
+  const double fvrr = 6.0 * (nmax + 1) * (mmax + 1);
+  double fh = 0.0;
+  for (int j = 1; j <= lb; ++j) fh += (double)(nmax - j + 1) * (mmax + 1);
+  for (int l = 1; l <= ld; ++l) fh += (double)(mmax - l + 1) * (la + 1) * (lb + 1);
+  const double fhrr = 2.0 * fh;
+  const double nc = (double)ncart(la) * ncart(lb) * ncart(lc) * ncart(ld);
+  const double kprod = (double)ka * kb * kc * kd;
+  if (!deriv) {
+    const double fprim = 60.0 + 56.0 * N + N * (25.0 + 3.0 * (fvrr + fhrr)) + 3.0 * N * nc;
+    const double nsa = nsph(la), nsb = nsph(lb), nsc = nsph(lc), nsd = nsph(ld);
+    const double nca = ncart(la), ncb = ncart(lb), ncc = ncart(lc), ncd = ncart(ld);
+    const double fc2s = 2.0 * (nsa * nca * ncb * ncc * ncd + nsa * nsb * ncb * ncc * ncd + nsa * nsb * nsc * ncc * ncd + nsa * nsb * nsc * nsd * ncd);
+    return kprod * fprim + fc2s + 12.0 * nsa * nsb * nsc * nsd;
+  }
+  // gradient: per root and element 3 pair products + 9 derivative FMAs; 18 density FMAs per element and primitive quartet
+  const double fprim = 60.0 + 56.0 * N + N * (25.0 + 3.0 * (fvrr + fhrr)) + 21.0 * N * nc + 36.0 * nc;
+  return kprod * fprim;
+}
+
+// dense-mode decomposition of one unit for a (BI, BJ) tile shape
+void make_rows(const std::vector<int>& count, int BI, int BJ, std::vector<int>& row_off) {
+  const int nb = (int)count.size(), nrows = (nb + BI - 1) / BI;
+  row_off.assign(nrows + 1, 0);
+  for (int r = 0; r < nrows; ++r) {
+    int mx = 0;
+    for (int i = r * BI; i < std::min(nb, (r + 1) * BI); ++i) mx = std::max(mx, count[i]);
+    row_off[r + 1] = row_off[r] + (mx + BJ - 1) / BJ;
+  }
+}
+
+int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
+  const PairClass& P = *pl.pcs[u.P]; const PairClass& R = *pl.pcs[u.R];
+  TunedInfo ti{};
+  u.kernel = 0; u.BI = GENERIC_BI; u.BJ = GENERIC_BJ;
+  const bool canonical = P.la >= P.lb && R.la >= R.lb && (P.la > R.la || (P.la == R.la && P.lb >= R.lb));
+  if (pl.kernel_mode == 0 && canonical && tuned_jk_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel = ti.kind; u.BI = ti.BI; u.BJ = ti.BJ; }
+  u.kernel_grad = 0; u.gBI = GENERIC_GRAD_BI; u.gBJ = GENERIC_GRAD_BJ;
+  if (pl.kernel_mode == 0 && canonical && tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = ti.kind; u.gBI = ti.BI; u.gBJ = ti.BJ; }
+  if (!pl.is_list) {
+    std::vector<int> ro;
+    make_rows(u.h_count, u.BI, u.BJ, ro);
+    u.nrows = (int)ro.size() - 1; u.nblocks = ro.back();
+    CK(u.row_off.upload(ro, s));
+    if (pl.want_grad) {
+      make_rows(u.h_count, u.gBI, u.gBJ, ro);
+      u.g_nrows = (int)ro.size() - 1; u.g_nblocks = ro.back();
+      CK(u.g_row_off.upload(ro, s));
+    }
+    CK(cudaStreamSynchronize(s));
+  }
+  return ERI_OK;
+}
+
+Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
+  Work w{};
+  w.bra = pl.pcs[u.P]->view(); w.ket = pl.pcs[u.R]->view();
+  w.ket_count = u.ket_count.p;
+  w.row_off = grad ? u.g_row_off.p : u.row_off.p;
+  w.nrows = grad ? u.g_nrows : u.nrows;
+  w.same = u.same ? 1 : 0;
+  w.list = pl.is_list ? u.list.p : nullptr; w.nlist = u.nlist;
+  w.rys = g_rys; w.D = pl.Dc.p; w.J = pl.Jc.p; w.K = pl.Kc.p; w.nao = pl.basis.nao_cart;
+  return w;
+}
+
+int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
+  for (auto& up : pl.units) {
+    Unit& u = *up;
+    Work w = make_work(pl, u, grad);
+    w.gJ = gJ; w.gK = gK;
+    if (pl.timing) CK(cudaEventRecord(pl.ev0, s));
+    if (!grad) {
+      if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s)); else CK(launch_tuned_jk(w, u.nblocks, s));
+    } else {
+      if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s)); else CK(launch_tuned_grad(w, u.g_nblocks, s));
+    }
+    if (pl.timing) {
+      CK(cudaEventRecord(pl.ev1, s)); CK(cudaEventSynchronize(pl.ev1));
+      float ms = 0; CK(cudaEventElapsedTime(&ms, pl.ev0, pl.ev1));
+      (grad ? u.last_ms_grad : u.last_ms) = ms;
+    }
+  }
+  return ERI_OK;
+}
+
+int plan_common(eri_plan& pl, const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim,
+                const double* coords, int natm, cudaStream_t s) {
+  CKI(make_basis(shells, nshell, prims, nprim, coords, natm, pl.basis));   // argument errors first: they need no device
+  CKI(ensure_init());
+  CKI(make_shell_map(pl, s));
+  CK(cudaEventCreate(&pl.ev0)); CK(cudaEventCreate(&pl.ev1));
+  return ERI_OK;
+}
+
+int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                      double thr, int want_grad, cudaStream_t s, eri_plan& pl) {
+  const auto t0 = std::chrono::steady_clock::now();
+  if (!(thr >= 0.0)) return fail(ERI_ERR_BAD_ARG, "schwarz_thr must be >= 0");
+  CKI(plan_common(pl, shells, nshell, prims, nprim, coords, natm, s));
+  pl.thr = thr; pl.want_grad = want_grad != 0;
+  const Basis& b = pl.basis;
+  const int ng = (int)b.groups.size();
+  // pair sets |ab, KaKb} for group(a) >= group(b) (groups sorted by (l,K), so la >= lb) -- Alg. 1 lines 3-6
+  std::vector<std::unique_ptr<PairClass>> all;
+  double qmax = 0.0;
+  long long pairs_total = 0;
+  for (int ga = 0; ga < ng; ++ga)
+    for (int gb = 0; gb <= ga; ++gb) {
+      auto pc = std::make_unique<PairClass>();
+      init_pair_class(b, ga, gb, *pc);
+      const auto& A = b.groups[ga].shells; const auto& B = b.groups[gb].shells;
+      for (size_t ia = 0; ia < A.size(); ++ia)
+        for (size_t ib = 0; ib < (ga == gb ? ia + 1 : B.size()); ++ib) {
+          pc->sa.push_back(A[ia]); pc->sb.push_back(B[ib]); pc->wgt.push_back(A[ia] == B[ib] ? 0.5 : 1.0);
+        }
+      pairs_total += (long long)pc->sa.size();
+      CKI(upload_pair_class(b, *pc, s));
+      CKI(schwarz_of_class(*pc, s));
+      for (double q : pc->Q) qmax = std::max(qmax, q);
+      all.push_back(std::move(pc));
+    }
+  // prescreen (Alg. 1 line 7), sort by decreasing bound (the paper bins, Eq. 6; sorting is the limit of fine bins)
+  long long pairs_kept = 0;
+  for (auto& pc : all) {
+    std::vector<int> idx;
+    for (int i = 0; i < pc->npair; ++i) if (thr == 0.0 || pc->Q[i] * qmax >= thr) idx.push_back(i);
+    std::stable_sort(idx.begin(), idx.end(), [&](int x, int y) { return pc->Q[x] > pc->Q[y]; });
+    if (idx.empty()) continue;
+    auto np = std::make_unique<PairClass>();
+    init_pair_class(b, pc->ga, pc->gb, *np);
+    for (int i : idx) { np->sa.push_back(pc->sa[i]); np->sb.push_back(pc->sb[i]); np->wgt.push_back(pc->wgt[i]); np->Q.push_back(pc->Q[i]); }
+    CKI(upload_pair_class(b, *np, s));
+    pairs_kept += np->npair;
+    pl.pcs.push_back(std::move(np));
+  }
+  all.clear();
+  // canonical order of pair sets: by (la, lb), then groups; bra set >= ket set gives (la,lb) >= (lc,ld)
+  std::sort(pl.pcs.begin(), pl.pcs.end(), [](const std::unique_ptr<PairClass>& x, const std::unique_ptr<PairClass>& y) {
+    return std::make_tuple(x->la, x->lb, x->ga, x->gb) < std::make_tuple(y->la, y->lb, y->ga, y->gb);
+  });
+  // work units: bra set P >= ket set R; per bra pair the kept kets are a prefix of the sorted ket set (reading R7)
+  long long qkept = 0; double flops = 0, flops_g = 0;
+  for (int P = 0; P < (int)pl.pcs.size(); ++P)
+    for (int R = 0; R <= P; ++R) {
+      const PairClass& bp = *pl.pcs[P]; const PairClass& kp = *pl.pcs[R];
+      auto u = std::make_unique<Unit>();
+      u->P = P; u->R = R; u->same = (P == R);
+      u->h_count.resize(bp.npair);
+      long long tot = 0;
+      for (int i = 0; i < bp.npair; ++i) {
+        int cnt = kp.npair;
+        if (thr > 0.0) {   // largest prefix with Q_i * Q_j >= thr
+          int lo = 0, hi = kp.npair;
+          while (lo < hi) { const int mid = (lo + hi) / 2; if (bp.Q[i] * kp.Q[mid] >= thr) lo = mid + 1; else hi = mid; }
+          cnt = lo;
+        }
+        if (u->same) cnt = std::min(cnt, i + 1);
+        u->h_count[i] = cnt; tot += cnt;
+      }
+      if (tot == 0) continue;
+      u->quartets = tot;
+      u->flops = tot * canonical_flops(bp.la, bp.lb, kp.la, kp.lb, bp.Ka, bp.Kb, kp.Ka, kp.Kb, 0);
+      u->flops_grad = tot * canonical_flops(bp.la, bp.lb, kp.la, kp.lb, bp.Ka, bp.Kb, kp.Ka, kp.Kb, 1);
+      CK(u->ket_count.upload(u->h_count, s));
+      CKI(select_kernels(pl, *u, s));
+      qkept += tot; flops += u->flops; flops_g += u->flops_grad;
+      pl.units.push_back(std::move(u));
+    }
+  CK(cudaStreamSynchronize(s));
+  eri_stats_t& st = pl.stats;
+  st.nshell = nshell; st.nao = b.nao; st.nao_cart = b.nao_cart; st.natm = natm;
+  st.n_shell_groups = ng; st.n_pair_classes = (int)pl.pcs.size(); st.n_quartet_classes = (int)pl.units.size();
+  st.launches_per_call = (int)pl.units.size() + 5;
+  st.pairs_total = pairs_total; st.pairs_kept = pairs_kept;
+  st.quartets_total = pairs_total * (pairs_total + 1) / 2; st.quartets_kept = qkept;
+  st.canonical_flops = flops; st.canonical_flops_grad = flops_g;
+  st.plan_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  return ERI_OK;
+}
+
+// list plan: pair sets from the distinct ordered shell pairs of the list, in the order given (any l order)
+int create_list_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                     const int32_t* quartets, int n, cudaStream_t s, eri_plan& pl, std::vector<long long>* cart_off_out,
+                     long long* cart_total) {
+  const auto t0 = std::chrono::steady_clock::now();
+  if (n < 0 || (n > 0 && !quartets)) return fail(ERI_ERR_BAD_ARG, "bad quartet list");
+  CKI(plan_common(pl, shells, nshell, prims, nprim, coords, natm, s));
+  pl.is_list = true;
+  const Basis& b = pl.basis;
+  for (int t = 0; t < 4 * n; ++t) if (quartets[t] < 0 || quartets[t] >= nshell) return fail(ERI_ERR_BAD_ARG, "quartet %d names shell %d", t / 4, quartets[t]);
+  std::map<std::pair<int, int>, int> class_of;            // (group, group) -> pair set index
+  std::vector<std::map<std::pair<int, int>, int>> pair_of;  // per pair set: (shell, shell) -> pair index
+  auto pair_id = [&](int i, int j, int& cls) {
+    const std::pair<int, int> key{b.group_of[i], b.group_of[j]};
+    auto it = class_of.find(key);
+    if (it == class_of.end()) {
+      it = class_of.emplace(key, (int)pl.pcs.size()).first;
+      auto pc = std::make_unique<PairClass>(); init_pair_class(b, key.first, key.second, *pc);
+      pl.pcs.push_back(std::move(pc)); pair_of.emplace_back();
+    }
+    cls = it->second;
+    auto& pm = pair_of[cls];
+    auto jt = pm.find({i, j});
+    if (jt == pm.end()) { jt = pm.emplace(std::make_pair(i, j), (int)pl.pcs[cls]->sa.size()).first; pl.pcs[cls]->sa.push_back(i); pl.pcs[cls]->sb.push_back(j); }
+    return jt->second;
+  };
+  std::map<std::pair<int, int>, int> unit_of;
+  std::vector<std::vector<int2>> lists; std::vector<std::vector<long long>> coffs;
+  long long ctot = 0;
+  if (cart_off_out) cart_off_out->resize(n);
+  double flops = 0;
+  for (int t = 0; t < n; ++t) {
+    int cb, ck;
+    const int pb = pair_id(quartets[4 * t], quartets[4 * t + 1], cb), pk = pair_id(quartets[4 * t + 2], quartets[4 * t + 3], ck);
+    auto it = unit_of.find({cb, ck});
+    if (it == unit_of.end()) {
+      it = unit_of.emplace(std::make_pair(cb, ck), (int)pl.units.size()).first;
+      auto u = std::make_unique<Unit>(); u->P = cb; u->R = ck; pl.units.push_back(std::move(u)); lists.emplace_back(); coffs.emplace_back();
+    }
+    lists[it->second].push_back(make_int2(pb, pk));
+    coffs[it->second].push_back(ctot);
+    if (cart_off_out) (*cart_off_out)[t] = ctot;
+    long long blk = 1; for (int x = 0; x < 4; ++x) blk *= ncart(b.sh[quartets[4 * t + x]].l);
+    ctot += blk;
+  }
+  if (cart_total) *cart_total = ctot;
+  for (auto& pc : pl.pcs) CKI(upload_pair_class(b, *pc, s));
+  for (size_t k = 0; k < pl.units.size(); ++k) {
+    Unit& u = *pl.units[k];
+    u.nlist = (int)lists[k].size(); u.quartets = u.nlist;
+    const PairClass& bp = *pl.pcs[u.P]; const PairClass& kp = *pl.pcs[u.R];
+    u.flops = u.quartets * canonical_flops(bp.la, bp.lb, kp.la, kp.lb, bp.Ka, bp.Kb, kp.Ka, kp.Kb, 0);
+    flops += u.flops;
+    CK(u.list.upload(lists[k], s));
+    if (cart_off_out) CK(u.coff.upload(coffs[k], s));
+    CKI(select_kernels(pl, u, s));
+  }
+  CK(cudaStreamSynchronize(s));
+  eri_stats_t& st = pl.stats;
+  st.nshell = nshell; st.nao = b.nao; st.nao_cart = b.nao_cart; st.natm = natm;
+  st.n_shell_groups = (int)b.groups.size(); st.n_pair_classes = (int)pl.pcs.size(); st.n_quartet_classes = (int)pl.units.size();
+  st.launches_per_call = (int)pl.units.size() + 5;
+  st.quartets_total = n; st.quartets_kept = n; st.canonical_flops = flops;
+  for (auto& pc : pl.pcs) { st.pairs_total += pc->npair; st.pairs_kept += pc->npair; }
+  st.plan_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  return ERI_OK;
+}
+
+int build_jk(eri_plan& pl, const double* D, double* J, double* K, cudaStream_t s) {
+  if (!D || !J || !K) return fail(ERI_ERR_BAD_ARG, "null matrix pointer");
+  const size_t n2 = (size_t)pl.basis.nao_cart * pl.basis.nao_cart;
+  if (pl.basis.nao == 0) return ERI_OK;
+  CK(launch_sph2cart(pl.map, D, pl.Dc.p, s));
+  CK(cudaMemsetAsync(pl.Jc.p, 0, n2 * sizeof(double), s));
+  CK(cudaMemsetAsync(pl.Kc.p, 0, n2 * sizeof(double), s));
+  CKI(run_units(pl, false, nullptr, nullptr, s));
+  if (pl.is_list) {
+    CK(launch_cart2sph(pl.map, pl.Jc.p, J, 1.0, 0, s));
+    CK(launch_cart2sph(pl.map, pl.Kc.p, K, 1.0, 0, s));
+  } else {   // reading R9: J = 2 (Jt + Jt^T), K = Kt + Kt^T
+    CK(launch_cart2sph(pl.map, pl.Jc.p, J, 2.0, 1, s));
+    CK(launch_cart2sph(pl.map, pl.Kc.p, K, 1.0, 1, s));
+  }
+  return ERI_OK;
+}
+
+int jk_grad(eri_plan& pl, const double* D, double* gJ, double* gK, cudaStream_t s) {
+  if (!D || !gJ || !gK) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  if (pl.is_list || !pl.want_grad) return fail(ERI_ERR_BAD_ARG, "plan was not created with want_grad");
+  if (pl.basis.natm == 0) return ERI_OK;
+  CK(cudaMemsetAsync(gJ, 0, sizeof(double) * 3 * pl.basis.natm, s));
+  CK(cudaMemsetAsync(gK, 0, sizeof(double) * 3 * pl.basis.natm, s));
+  if (pl.basis.nao == 0) return ERI_OK;
+  CK(launch_sph2cart(pl.map, D, pl.Dc.p, s));
+  return run_units(pl, true, gJ, gK, s);
+}
+
+}  // namespace
+}  // namespace eri
+
+// =================================================================================================================
+extern "C" {
+
+const char* eri_version(void) { return "liberi_b200 0.1 (sm_100a)"; }
+const char* eri_last_error(void) { return g_err.c_str(); }
+const char* eri_strerror(int code) {
+  switch (code) {
+    case ERI_OK: return "ok";
+    case ERI_ERR_BAD_ARG: return "bad argument";
+    case ERI_ERR_UNSUPPORTED_L: return "angular momentum outside 0..4";
+    case ERI_ERR_CUDA: return "CUDA failure";
+    case ERI_ERR_NOMEM: return "out of memory";
+    default: return "unknown error code";
+  }
+}
+
+double eri_canonical_flops(int la, int lb, int lc, int ld, int ka, int kb, int kc, int kd, int deriv) {
+  return canonical_flops(la, lb, lc, ld, ka, kb, kc, kd, deriv);
+}
+
+int eri_plan_create(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                    double schwarz_thr, int want_grad, void* stream, eri_plan_t** out) {
+  if (!out) return fail(ERI_ERR_BAD_ARG, "null out pointer");
+  *out = nullptr;
+  try {
+    auto pl = std::make_unique<eri_plan>();
+    CKI(create_dense_plan(shells, nshell, prims, nprim, coords, natm, schwarz_thr, want_grad, (cudaStream_t)stream, *pl));
+    *out = pl.release();
+    return ERI_OK;
+  } catch (const std::bad_alloc&) { return fail(ERI_ERR_NOMEM, "host allocation failed"); }
+    catch (...) { return fail(ERI_ERR_BAD_ARG, "unexpected exception"); }
+}
+
+int eri_list_plan_create(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                         const int32_t* quartets, int n, void* stream, eri_plan_t** out) {
+  if (!out) return fail(ERI_ERR_BAD_ARG, "null out pointer");
+  *out = nullptr;
+  try {
+    auto pl = std::make_unique<eri_plan>();
+    CKI(create_list_plan(shells, nshell, prims, nprim, coords, natm, quartets, n, (cudaStream_t)stream, *pl, nullptr, nullptr));
+    *out = pl.release();
+    return ERI_OK;
+  } catch (const std::bad_alloc&) { return fail(ERI_ERR_NOMEM, "host allocation failed"); }
+    catch (...) { return fail(ERI_ERR_BAD_ARG, "unexpected exception"); }
+}
+
+void eri_plan_destroy(eri_plan_t* plan) { delete plan; }
+
+int eri_plan_build_jk(eri_plan_t* plan, const double* D, double* J, double* K, void* stream) {
+  if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan");
+  if (plan->is_list) return fail(ERI_ERR_BAD_ARG, "list plan: use eri_list_plan_digest");
+  return build_jk(*plan, D, J, K, (cudaStream_t)stream);
+}
+int eri_list_plan_digest(eri_plan_t* plan, const double* D, double* Jt, double* Kt, void* stream) {
+  if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan");
+  if (!plan->is_list) return fail(ERI_ERR_BAD_ARG, "not a list plan");
+  return build_jk(*plan, D, Jt, Kt, (cudaStream_t)stream);
+}
+int eri_plan_jk_grad(eri_plan_t* plan, const double* D, double* gJ, double* gK, void* stream) {
+  if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan");
+  return jk_grad(*plan, D, gJ, gK, (cudaStream_t)stream);
+}
+
+int eri_plan_build_jk_host(eri_plan_t* plan, const double* D, double* J, double* K, void* stream) {
+  if (!plan || !D || !J || !K) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t n2 = (size_t)plan->basis.nao * plan->basis.nao;
+  if (plan->Dh.n != n2) { CK(plan->Dh.alloc(n2)); CK(plan->Jh.alloc(n2)); CK(plan->Kh.alloc(n2)); }
+  CK(cudaMemcpyAsync(plan->Dh.p, D, n2 * sizeof(double), cudaMemcpyHostToDevice, s));
+  CKI(plan->is_list ? eri_list_plan_digest(plan, plan->Dh.p, plan->Jh.p, plan->Kh.p, stream)
+                    : eri_plan_build_jk(plan, plan->Dh.p, plan->Jh.p, plan->Kh.p, stream));
+  CK(cudaMemcpyAsync(J, plan->Jh.p, n2 * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CK(cudaMemcpyAsync(K, plan->Kh.p, n2 * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  return ERI_OK;
+}
+
+int eri_plan_jk_grad_host(eri_plan_t* plan, const double* D, double* gJ, double* gK, void* stream) {
+  if (!plan || !D || !gJ || !gK) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t n2 = (size_t)plan->basis.nao * plan->basis.nao, ng = 3 * (size_t)plan->basis.natm;
+  if (plan->Dh.n != n2) { CK(plan->Dh.alloc(n2)); CK(plan->Jh.alloc(n2)); CK(plan->Kh.alloc(n2)); }
+  if (plan->gJd.n != ng) { CK(plan->gJd.alloc(ng)); CK(plan->gKd.alloc(ng)); }
+  CK(cudaMemcpyAsync(plan->Dh.p, D, n2 * sizeof(double), cudaMemcpyHostToDevice, s));
+  CKI(eri_plan_jk_grad(plan, plan->Dh.p, plan->gJd.p, plan->gKd.p, stream));
+  CK(cudaMemcpyAsync(gJ, plan->gJd.p, ng * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CK(cudaMemcpyAsync(gK, plan->gKd.p, ng * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  return ERI_OK;
+}
+
+int eri_plan_stats(const eri_plan_t* plan, eri_stats_t* out) {
+  if (!plan || !out) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  *out = plan->stats;
+  return ERI_OK;
+}
+int eri_plan_num_classes(const eri_plan_t* plan) { return plan ? (int)plan->units.size() : ERI_ERR_BAD_ARG; }
+int eri_plan_class_stats(const eri_plan_t* plan, eri_class_stat_t* out, int max_entries) {
+  if (!plan || (!out && max_entries > 0)) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  int k = 0;
+  for (const auto& up : plan->units) {
+    if (k >= max_entries) break;
+    const Unit& u = *up; const PairClass& P = *plan->pcs[u.P]; const PairClass& R = *plan->pcs[u.R];
+    eri_class_stat_t& c = out[k++];
+    c.la = P.la; c.lb = P.lb; c.lc = R.la; c.ld = R.lb; c.ka = P.Ka; c.kb = P.Kb; c.kc = R.Ka; c.kd = R.Kb;
+    c.nroots = (P.la + P.lb + R.la + R.lb) / 2 + 1; c.kernel = u.kernel; c.quartets = u.quartets;
+    c.canonical_flops = u.flops; c.last_ms = u.last_ms; c.last_ms_grad = u.last_ms_grad;
+  }
+  return k;
+}
+int eri_plan_set_timing(eri_plan_t* plan, int on) { if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan"); plan->timing = on; return ERI_OK; }
+int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode) {
+  if (!plan || mode < 0 || mode > 1) return fail(ERI_ERR_BAD_ARG, "bad kernel mode");
+  plan->kernel_mode = mode;
+  for (auto& u : plan->units) CKI(select_kernels(*plan, *u, nullptr));
+  return ERI_OK;
+}
+
+int eri_build_jk(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                 const double* D, double schwarz_thr, double* J, double* K, void* stream) {
+  eri_plan_t* pl = nullptr;
+  CKI(eri_plan_create(shells, nshell, prims, nprim, coords, natm, schwarz_thr, 0, stream, &pl));
+  int r = eri_plan_build_jk(pl, D, J, K, stream);
+  if (r == ERI_OK && cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) r = fail(ERI_ERR_CUDA, "stream synchronise failed");
+  eri_plan_destroy(pl);
+  return r;
+}
+
+int eri_jk_grad(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                const double* D, double schwarz_thr, double* gJ, double* gK, void* stream) {
+  eri_plan_t* pl = nullptr;
+  CKI(eri_plan_create(shells, nshell, prims, nprim, coords, natm, schwarz_thr, 1, stream, &pl));
+  int r = eri_plan_jk_grad(pl, D, gJ, gK, stream);
+  if (r == ERI_OK && cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) r = fail(ERI_ERR_CUDA, "stream synchronise failed");
+  eri_plan_destroy(pl);
+  return r;
+}
+
+int eri_digest_quartet_list(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                            const int32_t* quartets, int n, const double* D, double* Jt, double* Kt, void* stream) {
+  eri_plan_t* pl = nullptr;
+  CKI(eri_list_plan_create(shells, nshell, prims, nprim, coords, natm, quartets, n, stream, &pl));
+  int r = eri_list_plan_digest(pl, D, Jt, Kt, stream);
+  if (r == ERI_OK && cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) r = fail(ERI_ERR_CUDA, "stream synchronise failed");
+  eri_plan_destroy(pl);
+  return r;
+}
+
+int eri_compute_quartets(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                         const int32_t* quartets, int n, double* out, const int64_t* out_off, void* stream) {
+  if (n == 0) return ERI_OK;
+  if (!out || !out_off) return fail(ERI_ERR_BAD_ARG, "null output pointer");
+  cudaStream_t s = (cudaStream_t)stream;
+  try {
+    eri_plan pl;
+    std::vector<long long> coff; long long ctot = 0;
+    CKI(create_list_plan(shells, nshell, prims, nprim, coords, natm, quartets, n, s, pl, &coff, &ctot));
+    Dev<double> cart; CK(cart.alloc((size_t)ctot));
+    CK(cudaMemsetAsync(cart.p, 0, sizeof(double) * (size_t)ctot, s));
+    for (auto& up : pl.units) {
+      Work w = make_work(pl, *up, false);
+      CK(launch_generic_store(w, cart.p, up->coff.p, s));
+    }
+    std::vector<int> q4(quartets, quartets + 4 * (size_t)n);
+    std::vector<long long> ooff(out_off, out_off + n);
+    Dev<int> dq4; Dev<long long> dcoff, dooff;
+    CK(dq4.upload(q4, s)); CK(dcoff.upload(coff, s)); CK(dooff.upload(ooff, s));
+    CK(launch_block_c2s(pl.map, dq4.p, n, cart.p, dcoff.p, out, dooff.p, s));
+    CK(cudaStreamSynchronize(s));
+    return ERI_OK;
+  } catch (const std::bad_alloc&) { return fail(ERI_ERR_NOMEM, "host allocation failed"); }
+}
+
+int eri_schwarz(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
+                double* Q, void* stream) {
+  if (!Q && nshell > 0) return fail(ERI_ERR_BAD_ARG, "null output pointer");
+  cudaStream_t s = (cudaStream_t)stream;
+  try {
+    Basis b;
+    CKI(make_basis(shells, nshell, prims, nprim, coords, natm, b));
+    CKI(ensure_init());
+    const int ng = (int)b.groups.size();
+    for (int ga = 0; ga < ng; ++ga)
+      for (int gb = 0; gb <= ga; ++gb) {
+        PairClass pc; init_pair_class(b, ga, gb, pc);
+        for (int A : b.groups[ga].shells) for (int B : b.groups[gb].shells) { pc.sa.push_back(A); pc.sb.push_back(B); }
+        CKI(upload_pair_class(b, pc, s));
+        CKI(schwarz_of_class(pc, s));
+        for (int i = 0; i < pc.npair; ++i) Q[(size_t)pc.sa[i] * nshell + pc.sb[i]] = Q[(size_t)pc.sb[i] * nshell + pc.sa[i]] = pc.Q[i];
+      }
+    return ERI_OK;
+  } catch (const std::bad_alloc&) { return fail(ERI_ERR_NOMEM, "host allocation failed"); }
+}
+
+int eri_rys_roots(int nroots, const double* x, int n, double* u, double* w) {
+  if (nroots < 1 || nroots > RYS_NMAX) return fail(ERI_ERR_BAD_ARG, "nroots outside 1..%d", RYS_NMAX);
+  if (n < 0 || (n > 0 && (!x || !u || !w))) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  if (n == 0) return ERI_OK;
+  CKI(ensure_init());
+  Dev<double> dx, du, dw;
+  std::vector<double> hx(x, x + n);
+  CK(dx.upload(hx, nullptr)); CK(du.alloc((size_t)n * nroots)); CK(dw.alloc((size_t)n * nroots));
+  CK(launch_rys_diag(nroots, g_rys, dx.p, n, du.p, dw.p, nullptr));
+  CK(cudaMemcpy(u, du.p, sizeof(double) * n * nroots, cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(w, dw.p, sizeof(double) * n * nroots, cudaMemcpyDeviceToHost));
+  return ERI_OK;
+}
+
+int eri_c2s_matrix(int l, double* T) {   // diagnostic: the library's ns(l) x nc(l) table (reading R3)
+  if (l < 0 || l > LMAX || !T) return fail(ERI_ERR_BAD_ARG, "bad argument");
+  std::vector<double> t; build_c2s(l, t);
+  std::memcpy(T, t.data(), sizeof(double) * t.size());
+  return ERI_OK;
+}
+
+int eri_measure_fp64_peak(double* tflops, void* stream) {
+  if (!tflops) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  cudaStream_t s = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev)); CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  Dev<double> sink; CK(sink.alloc(1));
+  cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+  const int blocks = sms * 8, iters = 20000;
+  CK(launch_fp64_peak(sink.p, 2000, blocks, s));
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    CK(cudaEventRecord(e0, s)); CK(launch_fp64_peak(sink.p, iters, blocks, s)); CK(cudaEventRecord(e1, s));
+    CK(cudaEventSynchronize(e1));
+    float ms = 0; CK(cudaEventElapsedTime(&ms, e0, e1));
+    best = std::max(best, 2.0 * 16.0 * iters * 256.0 * blocks / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *tflops = best;
+  return ERI_OK;
+}
+
+}  // extern "C"

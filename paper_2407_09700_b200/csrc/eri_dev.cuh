@@ -1,0 +1,125 @@
+// eri_dev.cuh -- device-side data views and the Rys root/weight routine shared by all kernels of liberi_b200.
+// Product code (not test infrastructure); nothing under oracle/ is included, linked or called from here.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace eri {
+
+constexpr int LMAX = 4;
+constexpr double PI = 3.14159265358979323846;
+
+__host__ __device__ constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+__host__ __device__ constexpr int nsph(int l) { return 2 * l + 1; }
+__host__ __device__ constexpr int nroots_of(int L) { return L / 2 + 1; }  // Eq. 3
+
+// ---------------------------------------------------------------------------------------------------------------
+// Rys data buffer (one device allocation, read-only): see api.cu for how it is filled from rys_tables.inc.
+//   [0..16)    xmax[N]          switch to the Gauss-Hermite asymptote
+//   [16..32)   table offset[N]  (as double)
+//   [32..96)   h_n^2 of the 2N-point Gauss-Hermite rule, N-th block at 32 + N(N-1)/2
+//   [96..160)  v_n, same indexing
+//   [160..)    Chebyshev tables, per N: [interval][k=0..13][2N values]
+constexpr int RYS_HDR_XMAX = 0, RYS_HDR_OFF = 16, RYS_HDR_H2 = 32, RYS_HDR_V = 96, RYS_HDR_SIZE = 160;
+__host__ __device__ constexpr double rys_xmax(int N) {
+  return N == 1 ? 35.0 : N == 2 ? 45.0 : N == 3 ? 50.0 : N == 4 ? 57.5 : N == 5 ? 62.5 : N == 6 ? 67.5
+       : N == 7 ? 72.5 : N == 8 ? 77.5 : 82.5;
+}
+__host__ __device__ constexpr int rys_nint(int N) { return (int)(rys_xmax(N) / 2.5 + 0.5); }
+__host__ __device__ constexpr int rys_offset(int N) {  // doubles before the N-th table
+  int off = 0;
+  for (int n = 1; n < N; ++n) off += rys_nint(n) * 14 * 2 * n;
+  return off;
+}
+
+// Roots u_n = t_n^2 and weights w_n of the N-point rule for exp(-x t^2) on [0,1] (Eq. 1).
+// NN may be a compile-time constant (the loops unroll) or a run-time value.
+template <typename Int>
+__device__ __forceinline__ void rys_roots_impl(Int NN, int table_off, double xmax, double x,
+                                               const double* __restrict__ rys, double* u, double* w) {
+  const int N = NN;
+  if (x >= xmax) {
+    const double rx = 1.0 / x, rs = sqrt(rx);
+    const double* h2 = rys + RYS_HDR_H2 + N * (N - 1) / 2;
+    const double* v = rys + RYS_HDR_V + N * (N - 1) / 2;
+#pragma unroll
+    for (int n = 0; n < N; ++n) { u[n] = h2[n] * rx; w[n] = v[n] * rs; }
+    return;
+  }
+  int iv = (int)(x * 0.4);
+  const double s = (x - (2.5 * iv + 1.25)) * 0.8, s2 = 2.0 * s;
+  const double* c = rys + RYS_HDR_SIZE + table_off + iv * (28 * N);
+#pragma unroll
+  for (int n = 0; n < 2 * N; ++n) {
+    double b1 = c[13 * 2 * N + n], b2 = 0.0;
+#pragma unroll
+    for (int k = 12; k >= 1; --k) {
+      const double t = fma(s2, b1, c[k * 2 * N + n] - b2);
+      b2 = b1; b1 = t;
+    }
+    const double val = fma(s, b1, c[n] - b2);
+    if (n < N) u[n] = val; else w[n - N] = val;
+  }
+}
+
+template <int N>
+__device__ __forceinline__ void rys_roots(double x, const double* __restrict__ rys, double* u, double* w) {
+  rys_roots_impl<int>(N, rys_offset(N), rys_xmax(N), x, rys, u, w);
+}
+__device__ inline void rys_roots_rt(int N, double x, const double* __restrict__ rys, double* u, double* w) {
+  rys_roots_impl<int>(N, (int)rys[RYS_HDR_OFF + N], rys[RYS_HDR_XMAX + N], x, rys, u, w);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pair set |ab, KaKb}: all kept shell pairs of one (shell group, shell group) combination, sorted by
+// decreasing Schwarz factor.  SoA with the pair index fastest so that one-thread-per-quartet kernels coalesce.
+//   prim[(k*5 + f)*stride + i], f: 0 p = alpha+beta, 1..3 P = (alpha A + beta B)/p,
+//                               4 Kab = sqrt(2) pi^(5/4) / p * c_a c_b exp(-alpha beta / p |AB|^2)
+//   geom[f*stride + i], f: 0..2 A (centre of the first shell), 3..5 A - B, 6 pair weight (1/2 if both shells are the same)
+//   aexp[(k*2 + f)*stride + i], f: 0 alpha_a, 1 alpha_b            (gradient only)
+//   ao[i]   = (cartesian AO offset of first shell, of second shell);  atom[i] = (atom of first, of second)
+struct PairSet {
+  const double* prim;
+  const double* geom;
+  const double* aexp;
+  const double* q;   // Schwarz factor per pair, descending
+  const int2* ao;
+  const int2* atom;
+  int npair, stride, npp, la, lb;
+};
+
+// One (bra pair set, ket pair set) work unit.
+//  dense mode (list == nullptr): bra rows of BI pairs x ket blocks of BJ pairs; quartet (i,j) is evaluated iff
+//    j < ket_count[i] (prefix of the Schwarz-sorted ket set, already cut to j <= i when bra set == ket set).
+//    Block b belongs to the row r with row_off[r] <= b < row_off[r+1].
+//  list mode: work item t is the quartet (list[t].x, list[t].y); weight 1.
+struct Work {
+  PairSet bra, ket;
+  const int* ket_count;
+  const int* row_off;
+  int nrows;
+  int same;          // bra set == ket set: the diagonal quartet (i,i) carries another factor 1/2
+  const int2* list;
+  int nlist;
+  const double* rys;
+  const double* D;   // Cartesian-AO density, nao x nao
+  double* J;
+  double* K;
+  double* gJ;        // gradient accumulators, natm*3
+  double* gK;
+  int nao;
+};
+
+__device__ __forceinline__ void atomic_add(double* p, double v) { atomicAdd(p, v); }
+
+// locate the row of block b: largest r with row_off[r] <= b
+__device__ __forceinline__ int find_row(const int* __restrict__ row_off, int nrows, int b) {
+  int lo = 0, hi = nrows;  // row_off has nrows+1 entries
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (row_off[mid] <= b) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+}  // namespace eri

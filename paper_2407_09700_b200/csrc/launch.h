@@ -1,0 +1,41 @@
+// launch.h -- host-callable launchers of the kernel translation units of liberi_b200 (internal, not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include "eri_dev.cuh"
+
+namespace eri {
+
+// generic kernels: block = (GENERIC_BJ ket pairs) x (GENERIC_BI bra pairs), one thread per quartet
+constexpr int GENERIC_BJ = 32, GENERIC_BI = 4;
+constexpr int GENERIC_GRAD_BJ = 32, GENERIC_GRAD_BI = 4;
+
+cudaError_t launch_generic_jk(const Work& w, int nblocks_dense, cudaStream_t s);
+cudaError_t launch_generic_store(const Work& w, double* out, const long long* off, cudaStream_t s);
+cudaError_t launch_generic_grad(const Work& w, int nblocks_dense, cudaStream_t s);
+
+// tuned kernels: a launcher per l-class; returns false in `*handled` when the class has no tuned kernel.
+struct TunedInfo { int kind; int BI, BJ; };   // kind: 1 register-unrolled, 2 cooperative; tile shape for dense mode
+bool tuned_jk_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info);
+cudaError_t launch_tuned_jk(const Work& w, int nblocks_dense, cudaStream_t s);
+bool tuned_grad_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info);
+cudaError_t launch_tuned_grad(const Work& w, int nblocks_dense, cudaStream_t s);
+
+// transform.cu
+cudaError_t upload_c2s(const double* tables /*host, concatenated ns(l) x nc(l), l = 0..4*/);
+struct ShellMap {          // device arrays describing the AO layout
+  const int* sh_l; const int* sh_sph; const int* sh_cart;   // per shell
+  const int* sph2sh; const int* cart2sh;                    // per AO
+  int nshell, nao, nao_cart;
+};
+cudaError_t launch_sph2cart(const ShellMap& m, const double* Dsph, double* Dcart, cudaStream_t s);
+// out = T (alpha * (M + M^T if sym else M)) T^T
+cudaError_t launch_cart2sph(const ShellMap& m, const double* Mcart, double* Msph, double alpha, int sym, cudaStream_t s);
+// spherical blocks from Cartesian blocks: quartet t has shells q4[4t..4t+3], Cartesian block at cart + coff[t], output at out + ooff[t]
+cudaError_t launch_block_c2s(const ShellMap& m, const int* q4, int n, const double* cart, const long long* coff,
+                             double* out, const long long* ooff, cudaStream_t s);
+// Q[t] = sqrt(max_{s,t'} |(s t'|s t')|) over spherical components from the Cartesian block (ab|ab) [nab][nab] at cart + t*nab*nab
+cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, double* Q, cudaStream_t s);
+cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, double* u, double* w, cudaStream_t s);
+cudaError_t launch_fp64_peak(double* sink, int iters, int blocks, cudaStream_t s);
+
+}  // namespace eri

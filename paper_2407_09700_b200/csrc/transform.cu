@@ -1,0 +1,195 @@
+// transform.cu -- matrix-level Cartesian <-> real-solid-harmonic transforms (DESIGN.md step S5/S7), spherical
+// blocks for the diagnostic entry points, the Schwarz reduction (Eq. 7), and two small diagnostics.
+// The kernels digest in the Cartesian AO basis: D_cart = T^T D T once per call, J = T (2 (Jt + Jt^T)) T^T and
+// K = T (Kt + Kt^T) T^T at the end (reading R9) -- the paper never states how spherical functions are handled.
+#include "eri_dev.cuh"
+#include "launch.h"
+
+namespace eri {
+namespace {
+
+__constant__ double c_c2s[245];   // l-th table at c2s_off(l), ns(l) x nc(l) row-major
+__host__ __device__ constexpr int c2s_off(int l) { return l == 0 ? 0 : l == 1 ? 1 : l == 2 ? 10 : l == 3 ? 40 : 110; }
+
+__global__ void sph2cart_kernel(ShellMap m, const double* __restrict__ Ds, double* __restrict__ Dc) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long n2 = (long)m.nao_cart * m.nao_cart;
+  if (t >= n2) return;
+  const int p = (int)(t / m.nao_cart), q = (int)(t % m.nao_cart);
+  const int sp = m.cart2sh[p], sq = m.cart2sh[q];
+  const int lp = m.sh_l[sp], lq = m.sh_l[sq];
+  const int cp = p - m.sh_cart[sp], cq = q - m.sh_cart[sq];
+  const double* Tp = c_c2s + c2s_off(lp); const double* Tq = c_c2s + c2s_off(lq);
+  const int ncp = ncart(lp), ncq = ncart(lq);
+  const int p0 = m.sh_sph[sp], q0 = m.sh_sph[sq];
+  double acc = 0.0;
+  for (int a = 0; a < nsph(lp); ++a) {
+    const double ta = Tp[a * ncp + cp];
+    if (ta == 0.0) continue;
+    double row = 0.0;
+    for (int b = 0; b < nsph(lq); ++b) row += Ds[(long)(p0 + a) * m.nao + q0 + b] * Tq[b * ncq + cq];
+    acc += ta * row;
+  }
+  Dc[t] = acc;
+}
+
+__global__ void cart2sph_kernel(ShellMap m, const double* __restrict__ Mc, double* __restrict__ Ms, double alpha, int sym) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long n2 = (long)m.nao * m.nao;
+  if (t >= n2) return;
+  const int p = (int)(t / m.nao), q = (int)(t % m.nao);
+  const int sp = m.sph2sh[p], sq = m.sph2sh[q];
+  const int lp = m.sh_l[sp], lq = m.sh_l[sq];
+  const int a = p - m.sh_sph[sp], b = q - m.sh_sph[sq];
+  const int ncp = ncart(lp), ncq = ncart(lq);
+  const double* Tp = c_c2s + c2s_off(lp) + a * ncp; const double* Tq = c_c2s + c2s_off(lq) + b * ncq;
+  const int p0 = m.sh_cart[sp], q0 = m.sh_cart[sq];
+  const long n = m.nao_cart;
+  double acc = 0.0;
+  for (int cp = 0; cp < ncp; ++cp) {
+    if (Tp[cp] == 0.0) continue;
+    double row = 0.0;
+    for (int cq = 0; cq < ncq; ++cq) {
+      double v = Mc[(p0 + cp) * n + q0 + cq];
+      if (sym) v += Mc[(q0 + cq) * n + p0 + cp];
+      row += v * Tq[cq];
+    }
+    acc += Tp[cp] * row;
+  }
+  Ms[t] = alpha * acc;
+}
+
+// one block per quartet; four quarter transforms through shared memory would be faster, but this is a diagnostic path:
+// each thread forms one spherical element by the plain four-fold sum, skipping zero coefficients.
+__global__ void block_c2s_kernel(ShellMap m, const int* __restrict__ q4, const double* __restrict__ cart,
+                                 const long long* __restrict__ coff, double* __restrict__ out, const long long* __restrict__ ooff) {
+  const int t = blockIdx.x;
+  int l[4], nc[4], ns[4];
+  for (int x = 0; x < 4; ++x) { l[x] = m.sh_l[q4[4 * t + x]]; nc[x] = ncart(l[x]); ns[x] = nsph(l[x]); }
+  const double* src = cart + coff[t];
+  double* dst = out + ooff[t];
+  const int ntot = ns[0] * ns[1] * ns[2] * ns[3];
+  for (int e = threadIdx.x; e < ntot; e += blockDim.x) {
+    int r = e;
+    const int d = r % ns[3]; r /= ns[3];
+    const int c = r % ns[2]; r /= ns[2];
+    const int b = r % ns[1]; const int a = r / ns[1];
+    const double* Ta = c_c2s + c2s_off(l[0]) + a * nc[0];
+    const double* Tb = c_c2s + c2s_off(l[1]) + b * nc[1];
+    const double* Tc = c_c2s + c2s_off(l[2]) + c * nc[2];
+    const double* Td = c_c2s + c2s_off(l[3]) + d * nc[3];
+    double acc = 0.0;
+    for (int ia = 0; ia < nc[0]; ++ia) { if (Ta[ia] == 0.0) continue;
+      double sb = 0.0;
+      for (int ib = 0; ib < nc[1]; ++ib) { if (Tb[ib] == 0.0) continue;
+        double sc = 0.0;
+        for (int ic = 0; ic < nc[2]; ++ic) { if (Tc[ic] == 0.0) continue;
+          double sd = 0.0;
+          const double* row = src + (((long)ia * nc[1] + ib) * nc[2] + ic) * nc[3];
+          for (int id = 0; id < nc[3]; ++id) sd += Td[id] * row[id];
+          sc += Tc[ic] * sd;
+        }
+        sb += Tb[ib] * sc;
+      }
+      acc += Ta[ia] * sb;
+    }
+    dst[e] = acc;
+  }
+}
+
+// one warp per pair: spherical diagonal (st|st) from the Cartesian block M[(ab),(a'b')]
+__global__ void schwarz_diag_kernel(int la, int lb, int n, const double* __restrict__ cart, double* __restrict__ Q) {
+  const int t = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
+  const int lane = threadIdx.x % 32;
+  if (t >= n) return;
+  const int nca = ncart(la), ncb = ncart(lb), nab = nca * ncb;
+  const double* M = cart + (long)t * nab * nab;
+  const double* Ta = c_c2s + c2s_off(la); const double* Tb = c_c2s + c2s_off(lb);
+  double best = 0.0;
+  for (int st = lane; st < nsph(la) * nsph(lb); st += 32) {
+    const int s = st / nsph(lb), tt = st % nsph(lb);
+    double acc = 0.0;
+    for (int a = 0; a < nca; ++a) { const double ta = Ta[s * nca + a]; if (ta == 0.0) continue;
+      for (int b = 0; b < ncb; ++b) { const double tb = Tb[tt * ncb + b]; if (tb == 0.0) continue;
+        double inner = 0.0;
+        const double* row = M + (long)(a * ncb + b) * nab;
+        for (int a2 = 0; a2 < nca; ++a2) { const double ta2 = Ta[s * nca + a2]; if (ta2 == 0.0) continue;
+          for (int b2 = 0; b2 < ncb; ++b2) inner += ta2 * Tb[tt * ncb + b2] * row[a2 * ncb + b2];
+        }
+        acc += ta * tb * inner;
+      }
+    }
+    best = fmax(best, fabs(acc));
+  }
+  for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
+  if (lane == 0) Q[t] = sqrt(best);
+}
+
+__global__ void rys_diag_kernel(int N, const double* __restrict__ rys, const double* __restrict__ x, int n,
+                                double* __restrict__ u, double* __restrict__ w) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  double uu[9], ww[9];
+  rys_roots_rt(N, x[t], rys, uu, ww);
+  for (int k = 0; k < N; ++k) { u[(long)t * N + k] = uu[k]; w[(long)t * N + k] = ww[k]; }
+}
+
+// 16 independent FMA chains per thread; 2 flops per FMA
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double* sink, int iters) {
+  double a[16];
+  const double x = 1.0 + 1e-9 * threadIdx.x, y = 1e-9 * blockIdx.x;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = k * 0.125 + threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = fma(a[k], x, y);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k];
+  if (s == 123.456) sink[0] = s;   // never true; keeps the loop alive
+}
+
+}  // namespace
+
+cudaError_t upload_c2s(const double* tables) { return cudaMemcpyToSymbol(c_c2s, tables, sizeof(double) * 245); }
+
+cudaError_t launch_sph2cart(const ShellMap& m, const double* Ds, double* Dc, cudaStream_t s) {
+  const long n2 = (long)m.nao_cart * m.nao_cart;
+  if (n2 == 0) return cudaSuccess;
+  sph2cart_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, s>>>(m, Ds, Dc);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_cart2sph(const ShellMap& m, const double* Mc, double* Ms, double alpha, int sym, cudaStream_t s) {
+  const long n2 = (long)m.nao * m.nao;
+  if (n2 == 0) return cudaSuccess;
+  cart2sph_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, s>>>(m, Mc, Ms, alpha, sym);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_block_c2s(const ShellMap& m, const int* q4, int n, const double* cart, const long long* coff,
+                             double* out, const long long* ooff, cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  block_c2s_kernel<<<n, 128, 0, s>>>(m, q4, cart, coff, out, ooff);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, double* Q, cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  schwarz_diag_kernel<<<(n + 3) / 4, 128, 0, s>>>(la, lb, n, cart, Q);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, double* u, double* w, cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  rys_diag_kernel<<<(n + 127) / 128, 128, 0, s>>>(N, rys, x, n, u, w);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fp64_peak(double* sink, int iters, int blocks, cudaStream_t s) {
+  fp64_peak_kernel<<<blocks, 256, 0, s>>>(sink, iters);
+  return cudaGetLastError();
+}
+
+}  // namespace eri
