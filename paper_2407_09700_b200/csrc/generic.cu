@@ -21,8 +21,12 @@ struct QuartetGeom {
 //   I(0,0)=init; I(n+1,m) = C00 I(n,m) + n B10 I(n-1,m) + m B00 I(n,m-1); I(n,m+1) = C00' I(n,m) + m B01 I(n,m-1) + n B00 I(n-1,m)
 //   I(i,j+1,k,l) = I(i+1,j,k,l) + (A-B) I(i,j,k,l);  I(i,j,k,l+1) = I(i,j,k+1,l) + (C-D) I(i,j,k,l)
 // dims of the result: [na][nb][nc][nd] with na = la+1 (+raise) etc.; nmax = na+nb-2, mmax = nc+nd-2.
+// Numerical hygiene: the recurrence is built on the centre of the pair that is NEARER to
+// the product centre P (the one with the larger exponent) and transferred to the other one; the opposite order loses
+// up to (|AB|/|PB|)^l digits when a tight and a diffuse function sit several Bohr apart.  swap_bra: build on B,
+// transfer to A with (B-A); c00 must then be given relative to B.  Same for the ket.
 __device__ void fill_2d(double* __restrict__ G, int na, int nb, int nc, int nd, double init, double c00, double c00p,
-                        double b10, double b01, double b00, double ab, double cd) {
+                        double b10, double b01, double b00, double ab, double cd, bool swap_bra, bool swap_ket) {
   const int nmax = na + nb - 2, mmax = nc + nd - 2, M1 = mmax + 1;
   double T0[11 * 11];   // up to (l+1 raised): nmax, mmax <= 10
   double tmp[11 * 6];
@@ -36,22 +40,33 @@ __device__ void fill_2d(double* __restrict__ G, int na, int nb, int nc, int nd, 
       if (n > 0) v += n * b00 * T0[(n - 1) * M1 + m];
       T0[n * M1 + m + 1] = v;
     }
-  // bra transfer
+  // bra transfer: n1 = dimension of the centre the recurrence was built on, n2 = the other one
+  const int n1 = swap_bra ? nb : na, n2 = swap_bra ? na : nb;
+  const double x12 = swap_bra ? -ab : ab;
   for (int m = 0; m <= mmax; ++m) {
-    for (int i = 0; i <= nmax; ++i) tmp[i * nb] = T0[i * M1 + m];
-    for (int j = 1; j < nb; ++j)
-      for (int i = 0; i <= nmax - j; ++i) tmp[i * nb + j] = tmp[(i + 1) * nb + j - 1] + ab * tmp[i * nb + j - 1];
-    for (int i = 0; i < na; ++i)
-      for (int j = 0; j < nb; ++j) Bm[(i * nb + j) * M1 + m] = tmp[i * nb + j];
+    for (int i = 0; i <= nmax; ++i) tmp[i * n2] = T0[i * M1 + m];
+    for (int j = 1; j < n2; ++j)
+      for (int i = 0; i <= nmax - j; ++i) tmp[i * n2 + j] = tmp[(i + 1) * n2 + j - 1] + x12 * tmp[i * n2 + j - 1];
+    for (int i = 0; i < n1; ++i)
+      for (int j = 0; j < n2; ++j) Bm[(swap_bra ? j * nb + i : i * nb + j) * M1 + m] = tmp[i * n2 + j];
   }
   // ket transfer
+  const int m1 = swap_ket ? nd : nc, m2 = swap_ket ? nc : nd;
+  const double y12 = swap_ket ? -cd : cd;
   for (int ij = 0; ij < na * nb; ++ij) {
-    for (int k = 0; k <= mmax; ++k) tmp[k * nd] = Bm[ij * M1 + k];
-    for (int l = 1; l < nd; ++l)
-      for (int k = 0; k <= mmax - l; ++k) tmp[k * nd + l] = tmp[(k + 1) * nd + l - 1] + cd * tmp[k * nd + l - 1];
-    for (int k = 0; k < nc; ++k)
-      for (int l = 0; l < nd; ++l) G[(ij * nc + k) * nd + l] = tmp[k * nd + l];
+    for (int k = 0; k <= mmax; ++k) tmp[k * m2] = Bm[ij * M1 + k];
+    for (int l = 1; l < m2; ++l)
+      for (int k = 0; k <= mmax - l; ++k) tmp[k * m2 + l] = tmp[(k + 1) * m2 + l - 1] + y12 * tmp[k * m2 + l - 1];
+    for (int k = 0; k < m1; ++k)
+      for (int l = 0; l < m2; ++l) G[ij * nc * nd + (swap_ket ? l * nd + k : k * nd + l)] = tmp[k * m2 + l];
   }
+}
+
+// true if the second centre of the pair (B = A - AB) is nearer to the product centre P than the first one
+__device__ __forceinline__ bool swap_centre(const double* P, const double* A, const double* AB) {
+  double da = 0.0, db = 0.0;
+  for (int x = 0; x < 3; ++x) { const double pa = P[x] - A[x], pb = pa + AB[x]; da += pa * pa; db += pb * pb; }
+  return db < da;
 }
 
 // work item -> (bra pair i, ket pair j, weight); false if the thread has nothing to do
@@ -104,6 +119,7 @@ __device__ void quartet_loop(const Work& w, int i, int j, const QuartetGeom& g, 
       const double x = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
       const double pref = Kab * Kcd * sqrt(rpq);
       rys_roots_rt(N, x, w.rys, u, wt);
+      const bool swb = swap_centre(P, g.A, g.AB), swk = swap_centre(Q, g.C, g.CD);
       for (int r = 0; r < N; ++r) {
         const double t2 = u[r];
         const double b00 = 0.5 * t2 * rpq;
@@ -111,9 +127,9 @@ __device__ void quartet_loop(const Work& w, int i, int j, const QuartetGeom& g, 
         const double b01 = (1.0 - p * t2 * rpq) * 0.5 / q;
         double* G[3] = {gx, gy, gz};
         for (int ax = 0; ax < 3; ++ax) {
-          const double c00 = (P[ax] - g.A[ax]) - q * t2 * rpq * PQ[ax];
-          const double c00p = (Q[ax] - g.C[ax]) + p * t2 * rpq * PQ[ax];
-          fill_2d(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax]);
+          const double c00 = (P[ax] - g.A[ax]) + (swb ? g.AB[ax] : 0.0) - q * t2 * rpq * PQ[ax];
+          const double c00p = (Q[ax] - g.C[ax]) + (swk ? g.CD[ax] : 0.0) + p * t2 * rpq * PQ[ax];
+          fill_2d(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax], swb, swk);
         }
         cons(gx, gy, gz);
       }
@@ -187,7 +203,7 @@ __global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out,
 // and 18 accumulators (3 centres x 3 axes x {J,K}); 24 atomics at the end ("12 atomics per quartet").
 constexpr int GMAX1 = 6 * 6 * 6 * 5;
 
-__global__ void __launch_bounds__(64) generic_grad_kernel(Work w) {
+__global__ void __launch_bounds__(128) generic_grad_kernel(Work w) {
   int i, j; double f;
   if (!locate(w, i, j, f)) return;
   QuartetGeom g; load_geom(w, i, j, g);
@@ -218,6 +234,7 @@ __global__ void __launch_bounds__(64) generic_grad_kernel(Work w) {
       const double x = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
       const double pref = Kab * Kcd * sqrt(rpq);
       rys_roots_rt(N, x, w.rys, u, wt);
+      const bool swb = swap_centre(P, g.A, g.AB), swk = swap_centre(Q, g.C, g.CD);
       for (int r = 0; r < N; ++r) {
         const double t2 = u[r];
         const double b00 = 0.5 * t2 * rpq;
@@ -225,9 +242,9 @@ __global__ void __launch_bounds__(64) generic_grad_kernel(Work w) {
         const double b01 = (1.0 - p * t2 * rpq) * 0.5 / q;
         double* G[3] = {gx, gy, gz};
         for (int ax = 0; ax < 3; ++ax) {
-          const double c00 = (P[ax] - g.A[ax]) - q * t2 * rpq * PQ[ax];
-          const double c00p = (Q[ax] - g.C[ax]) + p * t2 * rpq * PQ[ax];
-          fill_2d(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax]);
+          const double c00 = (P[ax] - g.A[ax]) + (swb ? g.AB[ax] : 0.0) - q * t2 * rpq * PQ[ax];
+          const double c00p = (Q[ax] - g.C[ax]) + (swk ? g.CD[ax] : 0.0) + p * t2 * rpq * PQ[ax];
+          fill_2d(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax], swb, swk);
         }
         const int sa = nb * nc * nd, sb = nc * nd, sc = nd;
         for (int axx = la, ia = 0; axx >= 0; --axx) for (int ay = la - axx; ay >= 0; --ay, ++ia) { const int az = la - axx - ay;
