@@ -72,7 +72,7 @@ typedef struct {
   int32_t kernel;             /* 0 generic thread-per-quartet, 1 register-unrolled, 2 cooperative shared-memory */
   int64_t quartets;           /* kept unique quartets in this unit                             */
   double canonical_flops;     /* per call                                                      */
-  float last_ms;              /* device time of the unit's last launch; valid after eri_plan_set_timing(plan,1) */
+  float last_ms;              /* device time of the unit's last launch; needs eri_plan_set_timing(plan,1)      */
   float last_ms_grad;
 } eri_class_stat_t;
 
@@ -100,9 +100,15 @@ int eri_plan_jk_grad_host(eri_plan_t* plan, const double* D /*HOST*/, double* gr
 int eri_plan_stats(const eri_plan_t* plan, eri_stats_t* out);
 int eri_plan_num_classes(const eri_plan_t* plan);
 int eri_plan_class_stats(const eri_plan_t* plan, eri_class_stat_t* out /*HOST*/, int max_entries);
-int eri_plan_set_timing(eri_plan_t* plan, int on); /* bracket every class launch with CUDA events (serialises) */
+/* timing mode: a CUDA event is recorded on the stream between class launches (no host synchronisation); the per-class
+ * device times of the last call are collected by the next eri_plan_class_stats, which waits for that call to end. */
+int eri_plan_set_timing(eri_plan_t* plan, int on);
 /* kernel selection: 0 = tuned kernels where one exists (default), 1 = generic kernel everywhere (reference path) */
 int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode);
+/* Multi-GPU sharding: this process evaluates only the thread blocks b with b % nranks == rank of every
+ * class launch (quartets are independent units).  The outputs are then PARTIAL sums; J, K and the gradient
+ * are linear in them, so the caller sums the outputs over ranks (one all-reduce).  Default rank 0 of 1. */
+int eri_plan_set_shard(eri_plan_t* plan, int rank, int nranks);
 void eri_plan_destroy(eri_plan_t* plan);
 
 /* ---- diagnostics / benchmark entry points -------------------------------------------------------------------- */

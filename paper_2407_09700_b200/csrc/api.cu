@@ -231,7 +231,7 @@ int schwarz_of_class(PairClass& pc, cudaStream_t s) {
     for (int t = 0; t < m; ++t) { hl[t] = make_int2(start + t, start + t); ho[t] = (long long)t * blk; }
     CK(list.upload(hl, s)); CK(off.upload(ho, s));
     CK(cudaMemsetAsync(cart.p, 0, sizeof(double) * (size_t)m * blk, s));
-    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = list.p; w.nlist = m; w.rys = g_rys;
+    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = list.p; w.nlist = m; w.rys = g_rys; w.nshard = 1;
     CK(launch_generic_store(w, cart.p, off.p, s));
     CK(launch_schwarz_diag(pc.la, pc.lb, m, cart.p, qd.p, s));
     CK(cudaMemcpyAsync(pc.Q.data() + start, qd.p, sizeof(double) * m, cudaMemcpyDeviceToHost, s));
@@ -264,15 +264,16 @@ struct eri_plan {
   Basis basis;
   bool is_list = false, want_grad = false;
   double thr = 0.0;
-  int kernel_mode = 0, timing = 0;
+  int kernel_mode = 0, timing = 0, shard = 0, nshard = 1;
   std::vector<std::unique_ptr<PairClass>> pcs;
   std::vector<std::unique_ptr<Unit>> units;
   Dev<int> sh_l, sh_sph, sh_cart, sph2sh, cart2sh;
   Dev<double> Dc, Jc, Kc, Dh, Jh, Kh, gJd, gKd;   // Cartesian workspaces; device staging for the *_host entry points
   ShellMap map{};
   eri_stats_t stats{};
-  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-  ~eri_plan() { if (ev0) cudaEventDestroy(ev0); if (ev1) cudaEventDestroy(ev1); }
+  std::vector<cudaEvent_t> ev;   // timing mode: ev[k] before unit k, ev[n] after the last one (no host sync in between)
+  bool ev_pending = false, ev_grad = false;
+  ~eri_plan() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
 };
 
 namespace eri {
@@ -362,26 +363,24 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
   w.same = u.same ? 1 : 0;
   w.list = pl.is_list ? u.list.p : nullptr; w.nlist = u.nlist;
   w.rys = g_rys; w.D = pl.Dc.p; w.J = pl.Jc.p; w.K = pl.Kc.p; w.nao = pl.basis.nao_cart;
+  w.shard = pl.shard; w.nshard = pl.nshard;
   return w;
 }
 
 int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
+  if (pl.timing) while (pl.ev.size() < pl.units.size() + 1) { cudaEvent_t e; CK(cudaEventCreate(&e)); pl.ev.push_back(e); }
   for (auto& up : pl.units) {
     Unit& u = *up;
     Work w = make_work(pl, u, grad);
     w.gJ = gJ; w.gK = gK;
-    if (pl.timing) CK(cudaEventRecord(pl.ev0, s));
+    if (pl.timing) CK(cudaEventRecord(pl.ev[&up - &pl.units[0]], s));
     if (!grad) {
       if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s)); else CK(launch_tuned_jk(w, u.nblocks, s));
     } else {
       if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s)); else CK(launch_tuned_grad(w, u.g_nblocks, s));
     }
-    if (pl.timing) {
-      CK(cudaEventRecord(pl.ev1, s)); CK(cudaEventSynchronize(pl.ev1));
-      float ms = 0; CK(cudaEventElapsedTime(&ms, pl.ev0, pl.ev1));
-      (grad ? u.last_ms_grad : u.last_ms) = ms;
-    }
   }
+  if (pl.timing) { CK(cudaEventRecord(pl.ev[pl.units.size()], s)); pl.ev_pending = true; pl.ev_grad = grad; }
   return ERI_OK;
 }
 
@@ -390,7 +389,6 @@ int plan_common(eri_plan& pl, const eri_shell_t* shells, int nshell, const eri_p
   CKI(make_basis(shells, nshell, prims, nprim, coords, natm, pl.basis));   // argument errors first: they need no device
   CKI(ensure_init());
   CKI(make_shell_map(pl, s));
-  CK(cudaEventCreate(&pl.ev0)); CK(cudaEventCreate(&pl.ev1));
   return ERI_OK;
 }
 
@@ -627,6 +625,11 @@ int eri_list_plan_create(const eri_shell_t* shells, int nshell, const eri_prim_t
 }
 
 void eri_plan_destroy(eri_plan_t* plan) { delete plan; }
+int eri_plan_set_shard(eri_plan_t* plan, int rank, int nranks) {
+  if (!plan || nranks < 1 || rank < 0 || rank >= nranks) return fail(ERI_ERR_BAD_ARG, "bad shard %d of %d", rank, nranks);
+  plan->shard = rank; plan->nshard = nranks;
+  return ERI_OK;
+}
 
 int eri_plan_build_jk(eri_plan_t* plan, const double* D, double* J, double* K, void* stream) {
   if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan");
@@ -677,8 +680,18 @@ int eri_plan_stats(const eri_plan_t* plan, eri_stats_t* out) {
   return ERI_OK;
 }
 int eri_plan_num_classes(const eri_plan_t* plan) { return plan ? (int)plan->units.size() : ERI_ERR_BAD_ARG; }
-int eri_plan_class_stats(const eri_plan_t* plan, eri_class_stat_t* out, int max_entries) {
-  if (!plan || (!out && max_entries > 0)) return fail(ERI_ERR_BAD_ARG, "null pointer");
+int eri_plan_class_stats(const eri_plan_t* cplan, eri_class_stat_t* out, int max_entries) {
+  if (!cplan || (!out && max_entries > 0)) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  eri_plan_t* plan = const_cast<eri_plan_t*>(cplan);
+  if (plan->ev_pending) {   // collect the per-unit device times of the last timed call
+    const size_t n = plan->units.size();
+    CK(cudaEventSynchronize(plan->ev[n]));
+    for (size_t u = 0; u < n; ++u) {
+      float ms = 0; CK(cudaEventElapsedTime(&ms, plan->ev[u], plan->ev[u + 1]));
+      (plan->ev_grad ? plan->units[u]->last_ms_grad : plan->units[u]->last_ms) = ms;
+    }
+    plan->ev_pending = false;
+  }
   int k = 0;
   for (const auto& up : plan->units) {
     if (k >= max_entries) break;

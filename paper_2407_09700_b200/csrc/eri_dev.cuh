@@ -108,6 +108,7 @@ struct Work {
   double* gJ;        // gradient accumulators, natm*3
   double* gK;
   int nao;
+  int shard, nshard; // this process runs the blocks b = blockIdx.x * nshard + shard (eri_plan_set_shard)
 };
 
 __device__ __forceinline__ void atomic_add(double* p, double v) { atomicAdd(p, v); }

@@ -71,14 +71,16 @@ __device__ __forceinline__ bool swap_centre(const double* P, const double* A, co
 
 // work item -> (bra pair i, ket pair j, weight); false if the thread has nothing to do
 __device__ __forceinline__ bool locate(const Work& w, int& i, int& j, double& f) {
+  const int blk = blockIdx.x * w.nshard + w.shard;
   if (w.list) {
-    const long t = (long)blockIdx.x * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
+    const long t = (long)blk * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
     if (t >= w.nlist) return false;
     i = w.list[t].x; j = w.list[t].y; f = 1.0;
     return true;
   }
-  const int r = find_row(w.row_off, w.nrows, blockIdx.x);
-  const int jb = blockIdx.x - w.row_off[r];
+  if (blk >= w.row_off[w.nrows]) return false;
+  const int r = find_row(w.row_off, w.nrows, blk);
+  const int jb = blk - w.row_off[r];
   i = r * blockDim.y + threadIdx.y;
   j = jb * blockDim.x + threadIdx.x;
   if (i >= w.bra.npair) return false;
@@ -190,7 +192,7 @@ __global__ void __launch_bounds__(128) generic_jk_kernel(Work w) {
 __global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out, const long long* off) {
   int i, j; double f;
   if (!locate(w, i, j, f)) return;
-  const long t = (long)blockIdx.x * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
+  const long t = (long)(blockIdx.x * w.nshard + w.shard) * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
   QuartetGeom g; load_geom(w, i, j, g);
   StoreConsumer c{out + off[t], g.la, g.lb, g.lc, g.ld};
   quartet_loop(w, i, j, g, c);
@@ -287,7 +289,8 @@ __global__ void __launch_bounds__(128) generic_grad_kernel(Work w) {
 }  // namespace
 
 static int grid_of(const Work& w, int threads, int total_blocks_dense) {
-  return w.list ? (w.nlist + threads - 1) / threads : total_blocks_dense;
+  const int total = w.list ? (w.nlist + threads - 1) / threads : total_blocks_dense;
+  return (total + w.nshard - 1) / w.nshard;
 }
 
 cudaError_t launch_generic_jk(const Work& w, int nblocks_dense, cudaStream_t s) {

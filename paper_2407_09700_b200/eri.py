@@ -38,7 +38,7 @@ class eri_class_stat_t(ctypes.Structure):
 
 EXPORTS = ["eri_build_jk", "eri_jk_grad", "eri_plan_create", "eri_plan_build_jk", "eri_plan_jk_grad",
            "eri_plan_build_jk_host", "eri_plan_jk_grad_host", "eri_plan_stats", "eri_plan_num_classes",
-           "eri_plan_class_stats", "eri_plan_set_timing", "eri_plan_set_kernel_mode", "eri_plan_destroy",
+           "eri_plan_class_stats", "eri_plan_set_timing", "eri_plan_set_kernel_mode", "eri_plan_set_shard", "eri_plan_destroy",
            "eri_compute_quartets", "eri_digest_quartet_list", "eri_list_plan_create", "eri_list_plan_digest",
            "eri_schwarz", "eri_rys_roots", "eri_c2s_matrix", "eri_measure_fp64_peak", "eri_canonical_flops",
            "eri_strerror", "eri_last_error", "eri_version"]
@@ -68,6 +68,7 @@ def lib():
         L.eri_plan_class_stats.argtypes = [_vp, ctypes.POINTER(eri_class_stat_t), ctypes.c_int]
         L.eri_plan_set_timing.argtypes = [_vp, ctypes.c_int]
         L.eri_plan_set_kernel_mode.argtypes = [_vp, ctypes.c_int]
+        L.eri_plan_set_shard.argtypes = [_vp, ctypes.c_int, ctypes.c_int]
         _lib_handle = L
     return _lib_handle
 
@@ -164,6 +165,9 @@ class Plan:
 
     def set_kernel_mode(self, mode: int):
         _check(lib().eri_plan_set_kernel_mode(self._h, int(mode)))
+
+    def set_shard(self, rank: int, nranks: int):
+        _check(lib().eri_plan_set_shard(self._h, int(rank), int(nranks)))
 
 
 def eri_plan_create(basis, schwarz_thr: float, want_grad: bool = False) -> Plan:
