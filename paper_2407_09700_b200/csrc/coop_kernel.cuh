@@ -1,0 +1,350 @@
+// coop_kernel.cuh -- cooperative family of J/K kernels (family W).
+// One WARP per shell quartet.  The paper keeps the 2-D integrals of all roots of a quartet in per-thread local memory
+// (Algorithm 3) and is bound by local-memory traffic; here the 32 lanes share them
+// through shared memory:
+//   phase 1  lane (root r, axis x) builds I_x(i,j,k,l; t_r) -- vertical recurrence, then horizontal transfer on both
+//            sides at the 2-D level (reading R5), built on the centre nearer to P resp. Q
+//            -- and stores it to the warp's shared-memory slab S[axis][root][i][j][k][l];
+//   phase 2  lane `ab` owns the Cartesian bra component pair (a,b) (several per lane if nab > 32) and accumulates
+//            g[cd] = sum_r X Y Z for every ket component pair in registers (Eq. 1 and Eq. 5): per
+//            root 3 (lc+1)(ld+1) shared loads feed 2 nc(lc) nc(ld) FP64 operations;
+//   phase 3  contract-then-digest (the six updates of Alg. 2 lines 8-13) straight from registers:
+//            J_ab is complete per lane; K partial sums over d resp. c are formed per lane, summed over the lanes
+//            that share a resp. b through the (now dead) slab, and leave as one FP64 atomic per block element;
+//            J_cd is summed in registers over the bra pairs of the warp's task and reduced across lanes once per task.
+// A task is one ket pair and a run of CH consecutive bra pairs of the Schwarz-sorted tile row.
+#pragma once
+#include "eri_dev.cuh"
+#include "launch.h"
+
+namespace eri {
+
+constexpr int COOP_WARPS = 4;    // warps (= ket pairs) per block
+constexpr int COOP_CH = 16;      // bra pairs per task
+
+// one root of the N-point rule (same tables and asymptote as rys_roots_impl)
+template <int N>
+__device__ __forceinline__ void rys_root_one(double x, const double* __restrict__ rys, int r, double& u, double& w) {
+  if (x >= rys_xmax(N)) {
+    const double rx = 1.0 / x;
+    u = rys[RYS_HDR_H2 + N * (N - 1) / 2 + r] * rx;
+    w = rys[RYS_HDR_V + N * (N - 1) / 2 + r] * sqrt(rx);
+    return;
+  }
+  const int iv = (int)(x * 0.4);
+  const double s = (x - (2.5 * iv + 1.25)) * 0.8, s2 = 2.0 * s;
+  const double* c = rys + RYS_HDR_SIZE + rys_offset(N) + iv * (28 * N);
+  double b1u = c[13 * 2 * N + r], b2u = 0.0, b1w = c[13 * 2 * N + N + r], b2w = 0.0;
+#pragma unroll
+  for (int k = 12; k >= 1; --k) {
+    const double tu = fma(s2, b1u, c[k * 2 * N + r] - b2u), tw = fma(s2, b1w, c[k * 2 * N + N + r] - b2w);
+    b2u = b1u; b1u = tu; b2w = b1w; b1w = tw;
+  }
+  u = fma(s, b1u, c[r] - b2u);
+  w = fma(s, b1w, c[N + r] - b2w);
+}
+
+// 2-D integrals of one axis and one root, built on centres 1 (bra) and 3 (ket) and transferred to 2 and 4.
+// Element (i1,i2,i3,i4) is stored at dst[i1*s1 + i2*s2 + i3*s3 + i4*s4]; x12 = R1 - R2, x34 = R3 - R4.
+template <int L1, int L2, int L3, int L4>
+__device__ __forceinline__ void fill_2d_smem(double* __restrict__ dst, int s1, int s2, int s3, int s4, double init, double c00,
+                                             double c00p, double b10, double b01, double b00, double x12, double x34) {
+  constexpr int NM = L1 + L2, MM = L3 + L4;
+  double T[NM + 1][MM + 1];
+  T[0][0] = init;
+#pragma unroll
+  for (int n = 0; n < NM; ++n) T[n + 1][0] = n > 0 ? fma(c00, T[n][0], (n * b10) * T[n - 1][0]) : c00 * T[n][0];
+#pragma unroll
+  for (int m = 0; m < MM; ++m)
+#pragma unroll
+    for (int n = 0; n <= NM; ++n) {
+      double v = c00p * T[n][m];
+      if (m > 0) v = fma(m * b01, T[n][m - 1], v);
+      if (n > 0) v = fma(n * b00, T[n - 1][m], v);
+      T[n][m + 1] = v;
+    }
+  // bra transfer in place: after step j, T[i][m] (i <= NM - j) holds I(i, j, m)
+#pragma unroll
+  for (int j = 0; j <= L2; ++j) {
+    if (j > 0) {
+#pragma unroll
+      for (int i = 0; i <= NM - j; ++i)
+#pragma unroll
+        for (int m = 0; m <= MM; ++m) T[i][m] = fma(x12, T[i][m], T[i + 1][m]);
+    }
+    // ket transfer of the rows i <= L1 of this j, in place on a copy
+#pragma unroll
+    for (int i = 0; i <= L1; ++i) {
+      double R[MM + 1];
+#pragma unroll
+      for (int m = 0; m <= MM; ++m) R[m] = T[i][m];
+#pragma unroll
+      for (int l = 0; l <= L4; ++l) {
+        if (l > 0) {
+#pragma unroll
+          for (int k = 0; k <= MM - l; ++k) R[k] = fma(x34, R[k], R[k + 1]);
+        }
+#pragma unroll
+        for (int k = 0; k <= L3; ++k) dst[i * s1 + j * s2 + k * s3 + l * s4] = R[k];
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void cart_powers(int l, int k, int& lx, int& ly, int& lz) {
+  int row = 0;
+  while ((row + 1) * (row + 2) / 2 <= k) ++row;   // row = l - lx
+  lx = l - row;
+  ly = row - (k - row * (row + 1) / 2);
+  lz = l - lx - ly;
+}
+
+template <int LA, int LB, int LC, int LD>
+struct CoopTraits {
+  static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+  static constexpr int NAB = NA * NB, NCD = NC * ND;
+  static constexpr int PASSES = (NAB + 31) / 32;
+  static constexpr int N = nroots_of(LA + LB + LC + LD);
+  static constexpr int SCD = (LC + 1) * (LD + 1), G2 = (LA + 1) * (LB + 1) * SCD;
+  static constexpr int SLAB2D = 3 * N * G2;
+  static constexpr int KROW = (2 * (NC + ND)) | 1;           // per (a,b): Kac[NC] Kad[ND] Kbc[NC] Kbd[ND]; odd stride: no bank conflicts
+  static constexpr int SLABK = PASSES * 32 * KROW;
+  static constexpr int SLAB = (SLAB2D > SLABK ? SLAB2D : SLABK) + NCD;   // + staged D_cd
+  static constexpr size_t SMEM = sizeof(double) * SLAB * COOP_WARPS;
+};
+
+template <int LA, int LB, int LC, int LD>
+__global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
+  using Tr = CoopTraits<LA, LB, LC, LD>;
+  constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
+  constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2;
+  extern __shared__ double smem[];
+  const int lane = threadIdx.x, wy = threadIdx.y;
+  double* S = smem + (size_t)wy * Tr::SLAB;      // 2-D integrals, later the K partial sums
+  double* sDcd = S + (Tr::SLAB - NCD);             // D_cd of the task's ket pair
+
+  const PairSet& bp = w.bra; const PairSet& kp = w.ket;
+  const int blk = blockIdx.x * w.nshard + w.shard;
+  const bool list = w.list != nullptr;
+  int i_begin, i_end, j;
+  if (list) {
+    const long t = (long)blk * COOP_WARPS + wy;
+    if (t >= w.nlist) return;
+    i_begin = w.list[t].x; i_end = i_begin + 1; j = w.list[t].y;
+  } else {
+    if (blk >= w.row_off[w.nrows]) return;
+    const int r = find_row(w.row_off, w.nrows, blk);
+    j = (blk - w.row_off[r]) * COOP_WARPS + wy;
+    i_begin = r * COOP_CH; i_end = min(i_begin + COOP_CH, bp.npair);
+    if (j >= kp.npair) return;
+  }
+  const int n = w.nao;
+  const double* __restrict__ D = w.D;
+
+  // ---- per-task ket data ------------------------------------------------------------------------------------------
+  double C[3], CD[3];
+#pragma unroll
+  for (int x = 0; x < 3; ++x) { C[x] = kp.geom[x * kp.stride + j]; CD[x] = kp.geom[(3 + x) * kp.stride + j]; }
+  const double wket = kp.geom[6 * kp.stride + j];
+  const int c0 = kp.ao[j].x, d0 = kp.ao[j].y;
+  for (int cd = lane; cd < NCD; cd += 32) sDcd[cd] = D[(long)(c0 + cd / ND) * n + d0 + cd % ND];
+  __syncwarp();
+
+  // ---- per-lane roles ---------------------------------------------------------------------------------------------
+  // phase 1: lane -> (root, axis)
+  const int my_root = lane / 3, my_axis = lane - 3 * my_root;
+  const bool fill_lane = lane < 3 * N;
+  // phase 2: lane -> bra component pairs ab = lane + 32*pass
+  int offx[PASSES], offy[PASSES], offz[PASSES], ia[PASSES], ib[PASSES];
+#pragma unroll
+  for (int ps = 0; ps < PASSES; ++ps) {
+    int ab = lane + 32 * ps;
+    if (ab >= NAB) ab = NAB - 1;   // idle lanes of the last pass compute a duplicate that is never written out
+    ia[ps] = ab / NB; ib[ps] = ab - ia[ps] * NB;
+    int ax, ay, az, bx, by, bz;
+    cart_powers(LA, ia[ps], ax, ay, az); cart_powers(LB, ib[ps], bx, by, bz);
+    offx[ps] = (ax * (LB + 1) + bx) * SCD;
+    offy[ps] = (ay * (LB + 1) + by) * SCD + N * G2;
+    offz[ps] = (az * (LB + 1) + bz) * SCD + 2 * N * G2;
+  }
+  double pjcd[NCD];
+#pragma unroll
+  for (int cd = 0; cd < NCD; ++cd) pjcd[cd] = 0.0;
+
+  for (int i = i_begin; i < i_end; ++i) {
+    double f;
+    if (list) f = 1.0;
+    else {
+      if (j >= w.ket_count[i]) continue;     // warp-uniform
+      f = bp.geom[6 * bp.stride + i] * wket;
+      if (w.same && i == j) f *= 0.5;
+    }
+    double A[3], AB[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) { A[x] = bp.geom[x * bp.stride + i]; AB[x] = bp.geom[(3 + x) * bp.stride + i]; }
+    const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
+
+    double g[PASSES][NCD];
+#pragma unroll
+    for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+      for (int cd = 0; cd < NCD; ++cd) g[ps][cd] = 0.0;
+
+    for (int kb = 0; kb < bp.npp; ++kb) {
+      const double p = bp.prim[(kb * 5 + 0) * bp.stride + i];
+      const double P[3] = {bp.prim[(kb * 5 + 1) * bp.stride + i], bp.prim[(kb * 5 + 2) * bp.stride + i], bp.prim[(kb * 5 + 3) * bp.stride + i]};
+      const double Kab = bp.prim[(kb * 5 + 4) * bp.stride + i];
+      // build on B when P is nearer to B (only if there is something to transfer)
+      bool swb = false;
+      if (LB > 0) {
+        double da = 0.0, db = 0.0;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { const double pa = P[x] - A[x], pb = pa + AB[x]; da += pa * pa; db += pb * pb; }
+        swb = db < da;
+      }
+      for (int kk = 0; kk < kp.npp; ++kk) {
+        const double q = kp.prim[(kk * 5 + 0) * kp.stride + j];
+        const double Q[3] = {kp.prim[(kk * 5 + 1) * kp.stride + j], kp.prim[(kk * 5 + 2) * kp.stride + j], kp.prim[(kk * 5 + 3) * kp.stride + j]};
+        const double Kcd = kp.prim[(kk * 5 + 4) * kp.stride + j];
+        bool swk = false;
+        if (LD > 0) {
+          double dc = 0.0, dd = 0.0;
+#pragma unroll
+          for (int x = 0; x < 3; ++x) { const double qc = Q[x] - C[x], qd = qc + CD[x]; dc += qc * qc; dd += qd * qd; }
+          swk = dd < dc;
+        }
+        const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+        const double PQ[3] = {P[0] - Q[0], P[1] - Q[1], P[2] - Q[2]};
+        const double x = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
+        // ---- phase 1 ----
+        if (fill_lane) {
+          double u, wt;
+          rys_root_one<N>(x, w.rys, my_root, u, wt);
+          const double t2 = u * rpq;
+          const double b00 = 0.5 * t2, b10 = (1.0 - q * t2) * 0.5 / p, b01 = (1.0 - p * t2) * 0.5 / q;
+          const int ax = my_axis;
+          const double pa = (ax == 0 ? P[0] - A[0] : ax == 1 ? P[1] - A[1] : P[2] - A[2]);
+          const double qc = (ax == 0 ? Q[0] - C[0] : ax == 1 ? Q[1] - C[1] : Q[2] - C[2]);
+          const double pqx = (ax == 0 ? PQ[0] : ax == 1 ? PQ[1] : PQ[2]);
+          const double abx = (ax == 0 ? AB[0] : ax == 1 ? AB[1] : AB[2]);
+          const double cdx = (ax == 0 ? CD[0] : ax == 1 ? CD[1] : CD[2]);
+          const double c00 = pa + (swb ? abx : 0.0) - q * t2 * pqx;
+          const double c00p = qc + (swk ? cdx : 0.0) + p * t2 * pqx;
+          const double init = ax == 2 ? Kab * Kcd * sqrt(rpq) * wt : 1.0;
+          double* dst = S + (ax * N + my_root) * G2;
+          constexpr int SI = (LB + 1) * SCD, SJ = SCD, SK = LD + 1, SL = 1;
+          if (!swb) {
+            if (!swk) fill_2d_smem<LA, LB, LC, LD>(dst, SI, SJ, SK, SL, init, c00, c00p, b10, b01, b00, abx, cdx);
+            else if constexpr (LD > 0) fill_2d_smem<LA, LB, LD, LC>(dst, SI, SJ, SL, SK, init, c00, c00p, b10, b01, b00, abx, -cdx);
+          } else if constexpr (LB > 0) {
+            if (!swk) fill_2d_smem<LB, LA, LC, LD>(dst, SJ, SI, SK, SL, init, c00, c00p, b10, b01, b00, -abx, cdx);
+            else if constexpr (LD > 0) fill_2d_smem<LB, LA, LD, LC>(dst, SJ, SI, SL, SK, init, c00, c00p, b10, b01, b00, -abx, -cdx);
+          }
+        }
+        __syncwarp();
+        // ---- phase 2 ----
+#pragma unroll 1
+        for (int r = 0; r < N; ++r) {
+#pragma unroll
+          for (int ps = 0; ps < PASSES; ++ps) {
+            const double* X = S + offx[ps] + r * G2;
+            const double* Y = S + offy[ps] + r * G2;
+            const double* Z = S + offz[ps] + r * G2;
+            int cd = 0;
+#pragma unroll
+            for (int cx = LC; cx >= 0; --cx)
+#pragma unroll
+            for (int cy = LC - cx; cy >= 0; --cy)
+#pragma unroll
+            for (int dx = LD; dx >= 0; --dx)
+#pragma unroll
+            for (int dy = LD - dx; dy >= 0; --dy) {
+              const int cz = LC - cx - cy, dz = LD - dx - dy;
+              g[ps][cd] = fma(X[cx * (LD + 1) + dx] * Y[cy * (LD + 1) + dy], Z[cz * (LD + 1) + dz], g[ps][cd]);
+              ++cd;
+            }
+          }
+        }
+        __syncwarp();
+      }
+    }
+
+    // ---- phase 3: digestion ----------------------------------------------------------------------------------------
+#pragma unroll
+    for (int ps = 0; ps < PASSES; ++ps) {
+      const bool own = lane + 32 * ps < NAB;
+      const long ra = (long)(a0 + ia[ps]) * n, rb = (long)(b0 + ib[ps]) * n;
+      const double Dab = own ? f * D[ra + b0 + ib[ps]] : 0.0;
+      const double fo = own ? f : 0.0;
+      double Dac[NC], Dbc[NC], Dad[ND], Dbd[ND];
+#pragma unroll
+      for (int c = 0; c < NC; ++c) { Dac[c] = D[ra + c0 + c]; Dbc[c] = D[rb + c0 + c]; }
+#pragma unroll
+      for (int d = 0; d < ND; ++d) { Dad[d] = D[ra + d0 + d]; Dbd[d] = D[rb + d0 + d]; }
+      double jab = 0.0, kac[NC], kbc[NC], kad[ND], kbd[ND];
+#pragma unroll
+      for (int c = 0; c < NC; ++c) kac[c] = kbc[c] = 0.0;
+#pragma unroll
+      for (int d = 0; d < ND; ++d) kad[d] = kbd[d] = 0.0;
+#pragma unroll
+      for (int c = 0; c < NC; ++c)
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+          const double v = g[ps][c * ND + d];
+          jab = fma(v, sDcd[c * ND + d], jab);
+          pjcd[c * ND + d] = fma(v, Dab, pjcd[c * ND + d]);
+          kac[c] = fma(v, Dbd[d], kac[c]);
+          kad[d] = fma(v, Dbc[c], kad[d]);
+          kbc[c] = fma(v, Dad[d], kbc[c]);
+          kbd[d] = fma(v, Dac[c], kbd[d]);
+        }
+      if (own) atomic_add(w.J + ra + b0 + ib[ps], fo * jab);
+      double* row = S + (size_t)(lane + 32 * ps) * Tr::KROW;
+#pragma unroll
+      for (int c = 0; c < NC; ++c) { row[c] = fo * kac[c]; row[NC + ND + c] = fo * kbc[c]; }
+#pragma unroll
+      for (int d = 0; d < ND; ++d) { row[NC + d] = fo * kad[d]; row[2 * NC + ND + d] = fo * kbd[d]; }
+    }
+    __syncwarp();
+    // K_a. = sum over b of the rows (a,b); K_b. = sum over a.  Items: [a][NC+ND] then [b][NC+ND].
+    for (int it = lane; it < (NA + NB) * (NC + ND); it += 32) {
+      const bool isa = it < NA * (NC + ND);
+      const int rem = isa ? it : it - NA * (NC + ND);
+      const int s = rem / (NC + ND), e = rem - s * (NC + ND);    // s = a or b; e < NC: column c, else column d
+      double sum = 0.0;
+      if (isa) { for (int b = 0; b < NB; ++b) sum += S[(size_t)(s * NB + b) * Tr::KROW + e]; }
+      else     { for (int a = 0; a < NA; ++a) sum += S[(size_t)(a * NB + s) * Tr::KROW + (NC + ND) + e]; }
+      const long rowK = (long)((isa ? a0 : b0) + s) * n;
+      const int col = e < NC ? c0 + e : d0 + (e - NC);
+      atomic_add(w.K + rowK + col, sum);
+    }
+    __syncwarp();
+  }
+
+  // ---- J_cd of the task: sum the per-lane partial sums over the lanes ------------------------------------------------
+#pragma unroll
+  for (int cd = 0; cd < NCD; ++cd) {
+    double s = pjcd[cd];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == (cd & 31) && s != 0.0) atomic_add(w.J + (long)(c0 + cd / ND) * n + d0 + cd % ND, s);
+  }
+}
+
+template <int LA, int LB, int LC, int LD>
+cudaError_t launch_coop_jk(const Work& w, int nblocks_dense, cudaStream_t s) {
+  using Tr = CoopTraits<LA, LB, LC, LD>;
+  const int total = w.list ? (w.nlist + COOP_WARPS - 1) / COOP_WARPS : nblocks_dense;
+  const int grid = (total + w.nshard - 1) / w.nshard;
+  if (grid <= 0) return cudaSuccess;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(coop_jk_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  coop_jk_kernel<LA, LB, LC, LD><<<grid, dim3(32, COOP_WARPS), Tr::SMEM, s>>>(w);
+  return cudaGetLastError();
+}
+
+}  // namespace eri

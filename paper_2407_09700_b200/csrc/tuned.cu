@@ -1,10 +1,57 @@
-// tuned.cu -- dispatch table of the per-class tuned kernels (filled in by the reg_*.cu / coop_*.cu units).
+// tuned.cu -- dispatch table of the per-class tuned kernels: register family (reg_g*.cu), cooperative family (coop_*.cu).
 #include "launch.h"
+#include "reg_classes.h"
+#include "coop_classes.h"
 
 namespace eri {
 
-bool tuned_jk_info(int, int, int, int, int, int, TunedInfo*) { return false; }
-cudaError_t launch_tuned_jk(const Work&, int, cudaStream_t) { return cudaErrorNotSupported; }
+bool launch_reg_group0(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+bool launch_reg_group1(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+bool launch_reg_group2(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+bool launch_reg_group3(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+
+bool launch_coop_group0(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+bool launch_coop_group1(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+
+static bool is_coop_class(int key) {
+  switch (key) {
+#define X(a, b, c, d) case a * 1000 + b * 100 + c * 10 + d:
+    COOP_GROUP0(X) COOP_GROUP1(X)
+#undef X
+      return true;
+    default: return false;
+  }
+}
+
+static bool is_reg_class(int key) {
+  switch (key) {
+#define X(a, b, c, d) case a * 1000 + b * 100 + c * 10 + d:
+    REG_GROUP0(X) REG_GROUP1(X) REG_GROUP2(X) REG_GROUP3(X)
+#undef X
+      return true;
+    default: return false;
+  }
+}
+
+bool tuned_jk_info(int la, int lb, int lc, int ld, int, int, TunedInfo* info) {
+  const int key = la * 1000 + lb * 100 + lc * 10 + ld;
+  if (is_reg_class(key)) { info->kind = 1; info->BI = 4; info->BJ = 32; return true; }
+  if (is_coop_class(key)) { info->kind = 2; info->BI = 16; info->BJ = 4; return true; }   // COOP_CH bra pairs x COOP_WARPS ket pairs
+  return false;
+}
+
+cudaError_t launch_tuned_jk(const Work& w, int nblocks, cudaStream_t s) {
+  const int key = w.bra.la * 1000 + w.bra.lb * 100 + w.ket.la * 10 + w.ket.lb;
+  cudaError_t err = cudaErrorNotSupported;
+  if (launch_reg_group0(key, w, nblocks, s, &err)) return err;
+  if (launch_reg_group1(key, w, nblocks, s, &err)) return err;
+  if (launch_reg_group2(key, w, nblocks, s, &err)) return err;
+  if (launch_reg_group3(key, w, nblocks, s, &err)) return err;
+  if (launch_coop_group0(key, w, nblocks, s, &err)) return err;
+  if (launch_coop_group1(key, w, nblocks, s, &err)) return err;
+  return cudaErrorNotSupported;
+}
+
 bool tuned_grad_info(int, int, int, int, int, int, TunedInfo*) { return false; }
 cudaError_t launch_tuned_grad(const Work&, int, cudaStream_t) { return cudaErrorNotSupported; }
 
