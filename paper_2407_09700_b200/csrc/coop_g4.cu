@@ -1,12 +1,12 @@
-// coop_g1.cu -- instantiations of the cooperative-family J/K kernel for class group 1 (coop_classes.h).
+// coop_g4.cu -- instantiations of the cooperative-family J/K kernel for class group 4 (coop_classes.h).
 #include "coop_kernel.cuh"
 #include "coop_classes.h"
 
 namespace eri {
-bool launch_coop_group1(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err) {
+bool launch_coop_group4(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err) {
   switch (key) {
 #define X(a, b, c, d, tw) case a * 1000 + b * 100 + c * 10 + d: *err = launch_coop_jk<a, b, c, d, tw>(w, nblocks, s); return true;
-    COOP_GROUP1(X)
+    COOP_GROUP4(X)
 #undef X
     default: return false;
   }

@@ -13,6 +13,8 @@
 //            that share a resp. b through the (now dead) slab, and leave as one FP64 atomic per block element;
 //            J_cd is summed in registers over the bra pairs of the warp's task and reduced across lanes once per task.
 // A task is one ket pair and a run of CH consecutive bra pairs of the Schwarz-sorted tile row.
+// Large classes give a quartet to TW = 2 or 4 warps (a "group", synchronised with a named barrier) so that the
+// accumulators per lane, ceil(nab / 32 TW) * ncd, stay in registers.
 #pragma once
 #include "eri_dev.cuh"
 #include "launch.h"
@@ -99,27 +101,34 @@ __device__ __forceinline__ void cart_powers(int l, int k, int& lx, int& ly, int&
   lz = l - lx - ly;
 }
 
-template <int LA, int LB, int LC, int LD>
+__device__ __forceinline__ void group_sync(int tw, int id) {
+  if (tw == 1) __syncwarp();
+  else asm volatile("bar.sync %0, %1;" ::"r"(id + 1), "r"(32 * tw) : "memory");
+}
+
+template <int LA, int LB, int LC, int LD, int TW>
 struct CoopTraits {
+  static constexpr int T = 32 * TW, GROUPS = COOP_WARPS / TW;
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
   static constexpr int NAB = NA * NB, NCD = NC * ND;
-  static constexpr int PASSES = (NAB + 31) / 32;
+  static constexpr int PASSES = (NAB + T - 1) / T;
   static constexpr int N = nroots_of(LA + LB + LC + LD);
   static constexpr int SCD = (LC + 1) * (LD + 1), G2 = (LA + 1) * (LB + 1) * SCD;
   static constexpr int SLAB2D = 3 * N * G2;
   static constexpr int KROW = (2 * (NC + ND)) | 1;           // per (a,b): Kac[NC] Kad[ND] Kbc[NC] Kbd[ND]; odd stride: no bank conflicts
-  static constexpr int SLABK = PASSES * 32 * KROW;
+  static constexpr int SLABK = PASSES * T * KROW;
   static constexpr int SLAB = (SLAB2D > SLABK ? SLAB2D : SLABK) + NCD;   // + staged D_cd
-  static constexpr size_t SMEM = sizeof(double) * SLAB * COOP_WARPS;
+  static constexpr size_t SMEM = sizeof(double) * SLAB * GROUPS;
 };
 
-template <int LA, int LB, int LC, int LD>
+template <int LA, int LB, int LC, int LD, int TW>
 __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
-  using Tr = CoopTraits<LA, LB, LC, LD>;
+  using Tr = CoopTraits<LA, LB, LC, LD, TW>;
+  constexpr int T = Tr::T, GROUPS = Tr::GROUPS;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
   constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2;
   extern __shared__ double smem[];
-  const int lane = threadIdx.x, wy = threadIdx.y;
+  const int lane = threadIdx.x, wy = threadIdx.y;   // lane: thread within the group of T; wy: group within the block
   double* S = smem + (size_t)wy * Tr::SLAB;      // 2-D integrals, later the K partial sums
   double* sDcd = S + (Tr::SLAB - NCD);             // D_cd of the task's ket pair
 
@@ -128,13 +137,13 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
   const bool list = w.list != nullptr;
   int i_begin, i_end, j;
   if (list) {
-    const long t = (long)blk * COOP_WARPS + wy;
+    const long t = (long)blk * GROUPS + wy;
     if (t >= w.nlist) return;
     i_begin = w.list[t].x; i_end = i_begin + 1; j = w.list[t].y;
   } else {
     if (blk >= w.row_off[w.nrows]) return;
     const int r = find_row(w.row_off, w.nrows, blk);
-    j = (blk - w.row_off[r]) * COOP_WARPS + wy;
+    j = (blk - w.row_off[r]) * GROUPS + wy;
     i_begin = r * COOP_CH; i_end = min(i_begin + COOP_CH, bp.npair);
     if (j >= kp.npair) return;
   }
@@ -147,18 +156,18 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
   for (int x = 0; x < 3; ++x) { C[x] = kp.geom[x * kp.stride + j]; CD[x] = kp.geom[(3 + x) * kp.stride + j]; }
   const double wket = kp.geom[6 * kp.stride + j];
   const int c0 = kp.ao[j].x, d0 = kp.ao[j].y;
-  for (int cd = lane; cd < NCD; cd += 32) sDcd[cd] = D[(long)(c0 + cd / ND) * n + d0 + cd % ND];
-  __syncwarp();
+  for (int cd = lane; cd < NCD; cd += T) sDcd[cd] = D[(long)(c0 + cd / ND) * n + d0 + cd % ND];
+  group_sync(TW, wy);
 
   // ---- per-lane roles ---------------------------------------------------------------------------------------------
   // phase 1: lane -> (root, axis)
   const int my_root = lane / 3, my_axis = lane - 3 * my_root;
   const bool fill_lane = lane < 3 * N;
-  // phase 2: lane -> bra component pairs ab = lane + 32*pass
+  // phase 2: lane -> bra component pairs ab = lane + T*pass
   int offx[PASSES], offy[PASSES], offz[PASSES], ia[PASSES], ib[PASSES];
 #pragma unroll
   for (int ps = 0; ps < PASSES; ++ps) {
-    int ab = lane + 32 * ps;
+    int ab = lane + T * ps;
     if (ab >= NAB) ab = NAB - 1;   // idle lanes of the last pass compute a duplicate that is never written out
     ia[ps] = ab / NB; ib[ps] = ab - ia[ps] * NB;
     int ax, ay, az, bx, by, bz;
@@ -241,7 +250,7 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
             else if constexpr (LD > 0) fill_2d_smem<LB, LA, LD, LC>(dst, SJ, SI, SL, SK, init, c00, c00p, b10, b01, b00, -abx, -cdx);
           }
         }
-        __syncwarp();
+        group_sync(TW, wy);
         // ---- phase 2 ----
 #pragma unroll 1
         for (int r = 0; r < N; ++r) {
@@ -265,14 +274,14 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
             }
           }
         }
-        __syncwarp();
+        group_sync(TW, wy);
       }
     }
 
     // ---- phase 3: digestion ----------------------------------------------------------------------------------------
 #pragma unroll
     for (int ps = 0; ps < PASSES; ++ps) {
-      const bool own = lane + 32 * ps < NAB;
+      const bool own = lane + T * ps < NAB;
       const long ra = (long)(a0 + ia[ps]) * n, rb = (long)(b0 + ib[ps]) * n;
       const double Dab = own ? f * D[ra + b0 + ib[ps]] : 0.0;
       const double fo = own ? f : 0.0;
@@ -299,15 +308,15 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
           kbd[d] = fma(v, Dac[c], kbd[d]);
         }
       if (own) atomic_add(w.J + ra + b0 + ib[ps], fo * jab);
-      double* row = S + (size_t)(lane + 32 * ps) * Tr::KROW;
+      double* row = S + (size_t)(lane + T * ps) * Tr::KROW;
 #pragma unroll
       for (int c = 0; c < NC; ++c) { row[c] = fo * kac[c]; row[NC + ND + c] = fo * kbc[c]; }
 #pragma unroll
       for (int d = 0; d < ND; ++d) { row[NC + d] = fo * kad[d]; row[2 * NC + ND + d] = fo * kbd[d]; }
     }
-    __syncwarp();
+    group_sync(TW, wy);
     // K_a. = sum over b of the rows (a,b); K_b. = sum over a.  Items: [a][NC+ND] then [b][NC+ND].
-    for (int it = lane; it < (NA + NB) * (NC + ND); it += 32) {
+    for (int it = lane; it < (NA + NB) * (NC + ND); it += T) {
       const bool isa = it < NA * (NC + ND);
       const int rem = isa ? it : it - NA * (NC + ND);
       const int s = rem / (NC + ND), e = rem - s * (NC + ND);    // s = a or b; e < NC: column c, else column d
@@ -318,7 +327,7 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
       const int col = e < NC ? c0 + e : d0 + (e - NC);
       atomic_add(w.K + rowK + col, sum);
     }
-    __syncwarp();
+    group_sync(TW, wy);
   }
 
   // ---- J_cd of the task: sum the per-lane partial sums over the lanes ------------------------------------------------
@@ -327,23 +336,23 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
     double s = pjcd[cd];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (lane == (cd & 31) && s != 0.0) atomic_add(w.J + (long)(c0 + cd / ND) * n + d0 + cd % ND, s);
+    if ((lane & 31) == (cd & 31) && s != 0.0) atomic_add(w.J + (long)(c0 + cd / ND) * n + d0 + cd % ND, s);
   }
 }
 
-template <int LA, int LB, int LC, int LD>
+template <int LA, int LB, int LC, int LD, int TW>
 cudaError_t launch_coop_jk(const Work& w, int nblocks_dense, cudaStream_t s) {
-  using Tr = CoopTraits<LA, LB, LC, LD>;
-  const int total = w.list ? (w.nlist + COOP_WARPS - 1) / COOP_WARPS : nblocks_dense;
+  using Tr = CoopTraits<LA, LB, LC, LD, TW>;
+  const int total = w.list ? (w.nlist + Tr::GROUPS - 1) / Tr::GROUPS : nblocks_dense;
   const int grid = (total + w.nshard - 1) / w.nshard;
   if (grid <= 0) return cudaSuccess;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(coop_jk_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(coop_jk_kernel<LA, LB, LC, LD, TW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  coop_jk_kernel<LA, LB, LC, LD><<<grid, dim3(32, COOP_WARPS), Tr::SMEM, s>>>(w);
+  coop_jk_kernel<LA, LB, LC, LD, TW><<<grid, dim3(Tr::T, Tr::GROUPS), Tr::SMEM, s>>>(w);
   return cudaGetLastError();
 }
 

@@ -10,16 +10,19 @@ bool launch_reg_group1(int key, const Work& w, int nblocks, cudaStream_t s, cuda
 bool launch_reg_group2(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
 bool launch_reg_group3(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
 
-bool launch_coop_group0(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
-bool launch_coop_group1(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+#define DECL(g) bool launch_coop_group##g(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+DECL(0) DECL(1) DECL(2) DECL(3) DECL(4) DECL(5) DECL(6) DECL(7)
+#undef DECL
+static_assert(COOP_NGROUPS == 8, "tuned.cu lists eight cooperative groups");
+#define COOP_ALL(X) COOP_GROUP0(X) COOP_GROUP1(X) COOP_GROUP2(X) COOP_GROUP3(X) COOP_GROUP4(X) COOP_GROUP5(X) COOP_GROUP6(X) COOP_GROUP7(X)
 
-static bool is_coop_class(int key) {
+// warps per quartet of a cooperative class, 0 if the class is not served
+static int coop_tw(int key) {
   switch (key) {
-#define X(a, b, c, d) case a * 1000 + b * 100 + c * 10 + d:
-    COOP_GROUP0(X) COOP_GROUP1(X)
+#define X(a, b, c, d, tw) case a * 1000 + b * 100 + c * 10 + d: return tw;
+    COOP_ALL(X)
 #undef X
-      return true;
-    default: return false;
+    default: return 0;
   }
 }
 
@@ -36,7 +39,7 @@ static bool is_reg_class(int key) {
 bool tuned_jk_info(int la, int lb, int lc, int ld, int, int, TunedInfo* info) {
   const int key = la * 1000 + lb * 100 + lc * 10 + ld;
   if (is_reg_class(key)) { info->kind = 1; info->BI = 4; info->BJ = 32; return true; }
-  if (is_coop_class(key)) { info->kind = 2; info->BI = 16; info->BJ = 4; return true; }   // COOP_CH bra pairs x COOP_WARPS ket pairs
+  if (const int tw = coop_tw(key)) { info->kind = 2; info->BI = 16; info->BJ = 4 / tw; return true; }   // COOP_CH bra pairs x (COOP_WARPS / TW) ket pairs
   return false;
 }
 
@@ -47,8 +50,9 @@ cudaError_t launch_tuned_jk(const Work& w, int nblocks, cudaStream_t s) {
   if (launch_reg_group1(key, w, nblocks, s, &err)) return err;
   if (launch_reg_group2(key, w, nblocks, s, &err)) return err;
   if (launch_reg_group3(key, w, nblocks, s, &err)) return err;
-  if (launch_coop_group0(key, w, nblocks, s, &err)) return err;
-  if (launch_coop_group1(key, w, nblocks, s, &err)) return err;
+#define TRY(g) if (launch_coop_group##g(key, w, nblocks, s, &err)) return err;
+  TRY(0) TRY(1) TRY(2) TRY(3) TRY(4) TRY(5) TRY(6) TRY(7)
+#undef TRY
   return cudaErrorNotSupported;
 }
 
