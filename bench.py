@@ -271,14 +271,14 @@ def main():
             "clocks": clocks, "e2e": e2e, "gpu_launches": (st["launches_per_call"]) * args.steps, "roofline": roofline, "cpu_baseline": cb}
     if args.per_class:
         with open(args.per_class, "w") as f:
-            f.write("la lb lc ld ka kb kc kd N kernel quartets ms canonical_GFLOPs TFLOP/s pct_peak unit\n")
+            f.write("la lb lc ld ka kb kc kd N kernel quartets ms canonical_GFLOPs TFLOP/s pct_peak unit slots\n")
             for u, c in enumerate(classes):
                 c["unit"] = u
             for c in sorted(classes, key=lambda c: -c[key]):
                 fl = c["canonical_flops"] if kind != "grad" else 0.0
                 tf = fl / (c[key] * 1e-3) / 1e12 if c[key] > 0 else 0.0
                 f.write(f"{c['la']} {c['lb']} {c['lc']} {c['ld']} {c['ka']} {c['kb']} {c['kc']} {c['kd']} {c['nroots']} {c['kernel']} "
-                        f"{c['quartets']} {c[key]:.4f} {fl / 1e9:.3f} {tf:.3f} {100 * tf / fp64_peak:.2f} {c['unit']}\n")
+                        f"{c['quartets']} {c[key]:.4f} {fl / 1e9:.3f} {tf:.3f} {100 * tf / fp64_peak:.2f} {c['unit']} {c['slots']}\n")
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -69,8 +69,9 @@ typedef struct {
   int32_t la, lb, lc, ld;     /* la >= lb, lc >= ld                                            */
   int32_t ka, kb, kc, kd;     /* contraction degrees                                           */
   int32_t nroots;             /* Eq. 3                                            */
-  int32_t kernel;             /* 0 generic thread-per-quartet, 1 register-unrolled, 2 cooperative shared-memory */
+  int32_t kernel;             /* 0 generic thread-per-quartet, 1 register-unrolled, 2 cooperative shared-memory, 3 tile */
   int64_t quartets;           /* kept unique quartets in this unit                             */
+  int64_t slots;              /* quartet slots the unit's J/K launch covers (tile shape x blocks) >= quartets: lane efficiency */
   double canonical_flops;     /* per call                                                      */
   float last_ms;              /* device time of the unit's last launch; needs eri_plan_set_timing(plan,1)      */
   float last_ms_grad;
@@ -103,7 +104,8 @@ int eri_plan_class_stats(const eri_plan_t* plan, eri_class_stat_t* out /*HOST*/,
 /* timing mode: a CUDA event is recorded on the stream between class launches (no host synchronisation); the per-class
  * device times of the last call are collected by the next eri_plan_class_stats, which waits for that call to end. */
 int eri_plan_set_timing(eri_plan_t* plan, int on);
-/* kernel selection: 0 = tuned kernels where one exists (default), 1 = generic kernel everywhere (reference path) */
+/* kernel selection: 0 = tuned kernels where one exists, tile family preferred (default), 1 = generic kernel everywhere
+ * (reference path), 2 = tuned kernels without the tile family (register and cooperative families only) */
 int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode);
 /* Multi-GPU sharding: this process evaluates only the thread blocks b with b % nranks == rank of every
  * class launch (quartets are independent units).  The outputs are then PARTIAL sums; J, K and the gradient

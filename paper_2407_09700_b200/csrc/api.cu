@@ -168,6 +168,12 @@ struct PairClass {
   std::vector<double> Q, wgt;    // Schwarz factor, pair weight
   Dev<double> prim, geom, aexp, q;
   Dev<int2> ao, atom;
+  // tile family: the same pairs in chunks of 32 slots that share the first shell (padding slots have Q = -1);
+  // chunks are ordered by decreasing largest Schwarz factor, which is the factor of the chunk's first slot
+  std::unique_ptr<PairClass> grouped;
+  std::vector<double> chunk_q;     // grouped only: largest Schwarz factor of each chunk (chunks are sorted by it, descending)
+  double fill = 0.0;               // grouped only: valid slots / slots
+  double hrr_loss = 1.0;           // max over primitive pairs of ((alpha_a + alpha_b) / alpha_a)^lb, see DESIGN.md "HRR direction"
   PairSet view() const {
     PairSet v; v.prim = prim.p; v.geom = geom.p; v.aexp = aexp.p; v.q = q.p; v.ao = ao.p; v.atom = atom.p;
     v.npair = npair; v.stride = stride; v.npp = npp; v.la = la; v.lb = lb; return v;
@@ -211,6 +217,51 @@ int upload_pair_class(const Basis& b, PairClass& pc, cudaStream_t s) {
   return ERI_OK;
 }
 
+// digits lost by the horizontal transfer when the 2-D integrals are built on the FIRST centre: |AB| / |PB| = p / alpha_a per quantum
+double hrr_loss_of(const Basis& b, const PairClass& pc) {
+  if (pc.lb == 0) return 1.0;
+  double worst = 1.0;
+  for (size_t i = 0; i < pc.sa.size(); ++i) {
+    const eri_shell_t& A = b.sh[pc.sa[i]]; const eri_shell_t& B = b.sh[pc.sb[i]];
+    if (A.atom == B.atom) continue;   // AB = 0: the transfer adds nothing
+    for (int ka = 0; ka < A.nprim; ++ka)
+      for (int kb = 0; kb < B.nprim; ++kb) {
+        const double ea = b.pr[A.prim_off + ka].exp, eb = b.pr[B.prim_off + kb].exp;
+        worst = std::max(worst, std::pow((ea + eb) / ea, pc.lb));
+      }
+  }
+  return worst;
+}
+
+void init_pair_class(const Basis& b, int ga, int gb, PairClass& pc);
+
+// grouped twin of a Schwarz-sorted pair set (tile family): every first shell's partner list (sorted by decreasing Q) is cut
+// into chunks of 32 slots, the chunks are sorted by their head's Q; padding slots have Q = -1.
+int make_grouped(const Basis& b, PairClass& pc, cudaStream_t s) {
+  auto gp = std::make_unique<PairClass>();
+  init_pair_class(b, pc.ga, pc.gb, *gp);
+  std::map<int, std::vector<int>> by_first;
+  for (int i = 0; i < pc.npair; ++i) by_first[pc.sa[i]].push_back(i);   // pc is sorted by decreasing Q, so is every group
+  struct Chunk { double q; const std::vector<int>* idx; int begin, n; };
+  std::vector<Chunk> chunks;
+  for (auto& kv : by_first)
+    for (int st = 0; st < (int)kv.second.size(); st += 32)
+      chunks.push_back(Chunk{pc.Q[kv.second[st]], &kv.second, st, std::min(32, (int)kv.second.size() - st)});
+  std::stable_sort(chunks.begin(), chunks.end(), [](const Chunk& x, const Chunk& y) { return x.q > y.q; });
+  for (const Chunk& c : chunks) {
+    gp->chunk_q.push_back(c.q);
+    for (int t = 0; t < 32; ++t) {
+      const int src = (*c.idx)[c.begin + (t < c.n ? t : 0)];   // padding repeats the chunk's first pair (valid addresses)
+      gp->sa.push_back(pc.sa[src]); gp->sb.push_back(pc.sb[src]); gp->wgt.push_back(pc.wgt[src]);
+      gp->Q.push_back(t < c.n ? pc.Q[src] : -1.0);
+    }
+  }
+  gp->fill = chunks.empty() ? 0.0 : (double)pc.npair / (32.0 * chunks.size());
+  CKI(upload_pair_class(b, *gp, s));
+  pc.grouped = std::move(gp);
+  return ERI_OK;
+}
+
 void init_pair_class(const Basis& b, int ga, int gb, PairClass& pc) {
   pc.ga = ga; pc.gb = gb; pc.la = b.groups[ga].l; pc.lb = b.groups[gb].l; pc.Ka = b.groups[ga].K; pc.Kb = b.groups[gb].K;
   pc.npp = pc.Ka * pc.Kb;
@@ -241,6 +292,9 @@ int schwarz_of_class(PairClass& pc, cudaStream_t s) {
 }
 
 // ---- work units -----------------------------------------------------------------------------------------------
+constexpr double TILE_MIN_FILL = 0.3;   // tile family only where at least this fraction of the swept lanes has work
+constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
+
 struct Unit {
   int P = 0, R = 0; bool same = false;
   int BI = GENERIC_BI, BJ = GENERIC_BJ, nrows = 0, nblocks = 0;
@@ -251,6 +305,7 @@ struct Unit {
   float last_ms = 0, last_ms_grad = 0;
   std::vector<int> h_count;
   Dev<int> ket_count, row_off, g_row_off;
+  Dev<int> t_row_slot, t_row_off; int t_nrows = 0, t_nblocks = 0, tBI = 0; long long t_slots = 0;   // tile family
   Dev<int2> list; int nlist = 0;            // list mode
   Dev<long long> coff;                      // list mode, store kernel
 };
@@ -336,7 +391,40 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
   TunedInfo ti{};
   u.kernel = 0; u.BI = GENERIC_BI; u.BJ = GENERIC_BJ;
   const bool canonical = P.la >= P.lb && R.la >= R.lb && (P.la > R.la || (P.la == R.la && P.lb >= R.lb));
-  if (pl.kernel_mode == 0 && canonical && tuned_jk_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel = ti.kind; u.BI = ti.BI; u.BJ = ti.BJ; }
+  if (pl.kernel_mode != 1 && canonical && tuned_jk_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel = ti.kind; u.BI = ti.BI; u.BJ = ti.BJ; }
+  // tile family: dense mode, and only where building the 2-D integrals on the first centre of every pair is safe
+  if (pl.kernel_mode == 0 && canonical && !pl.is_list && P.grouped && R.grouped && P.hrr_loss <= HRR_LOSS_MAX && R.hrr_loss <= HRR_LOSS_MAX &&
+      tile_jk_info(P.la, P.lb, R.la, R.lb, &ti)) {
+    const PairClass& gb = *P.grouped; const PairClass& gk = *R.grouped;
+    const int nbc = (int)gb.chunk_q.size(), nkc = (int)gk.chunk_q.size();
+    std::vector<int> slot, off{0};
+    long long slots = 0;
+    std::vector<double> rq(32);
+    for (int cb = 0; cb < nbc; ++cb) {   // one block per (bra chunk, ket chunk of the prefix that passes Schwarz)
+      const double qb = gb.chunk_q[cb];
+      int lo = 0, hi = nkc;
+      if (pl.thr > 0.0) { while (lo < hi) { const int mid = (lo + hi) / 2; if (qb * gk.chunk_q[mid] >= pl.thr) lo = mid + 1; else hi = mid; } }
+      else lo = nkc;
+      if (u.same) lo = std::min(lo, cb + 1);
+      if (lo == 0) continue;
+      slot.push_back(32 * cb); off.push_back(off.back() + lo);
+      // lane slots actually swept = rows with work x 32 (the kernel skips the other rows)
+      for (int y = 0; y < 32; ++y) rq[y] = gb.Q[32 * cb + y];
+      std::sort(rq.begin(), rq.end(), std::greater<double>());
+      for (int ck = 0; ck < lo; ++ck) {
+        int n = 0;
+        while (n < 32 && rq[n] >= 0.0 && rq[n] * gk.chunk_q[ck] >= pl.thr) ++n;
+        slots += 32 * n;
+      }
+    }
+    if (slots > 0 && (double)u.quartets / (double)slots >= TILE_MIN_FILL) {
+      if (getenv("ERI_DEBUG_UNITS")) fprintf(stderr, "UNIT %d %d %d %d %d %d %d %d eff %.3f brafill %.3f ketfill %.3f\n", P.la, P.lb, R.la, R.lb, P.Ka, P.Kb, R.Ka, R.Kb,
+                                           (double)u.quartets / (double)slots, gb.fill, gk.fill);
+      u.kernel = 3; u.tBI = ti.BI; u.t_slots = slots;
+      u.t_nrows = (int)slot.size(); u.t_nblocks = off.back();
+      CK(u.t_row_slot.upload(slot, s)); CK(u.t_row_off.upload(off, s));
+    }
+  }
   u.kernel_grad = 0; u.gBI = GENERIC_GRAD_BI; u.gBJ = GENERIC_GRAD_BJ;
   if (pl.kernel_mode == 0 && canonical && tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = ti.kind; u.gBI = ti.BI; u.gBJ = ti.BJ; }
   if (!pl.is_list) {
@@ -360,6 +448,11 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
   w.ket_count = u.ket_count.p;
   w.row_off = grad ? u.g_row_off.p : u.row_off.p;
   w.nrows = grad ? u.g_nrows : u.nrows;
+  w.thr = pl.thr;
+  if (!grad && u.kernel == 3) {
+    w.bra = pl.pcs[u.P]->grouped->view(); w.ket = pl.pcs[u.R]->grouped->view();
+    w.row_off = u.t_row_off.p; w.row_slot = u.t_row_slot.p; w.nrows = u.t_nrows;
+  }
   w.same = u.same ? 1 : 0;
   w.list = pl.is_list ? u.list.p : nullptr; w.nlist = u.nlist;
   w.rys = g_rys; w.D = pl.Dc.p; w.J = pl.Jc.p; w.K = pl.Kc.p; w.nao = pl.basis.nao_cart;
@@ -375,7 +468,9 @@ int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
     w.gJ = gJ; w.gK = gK;
     if (pl.timing) CK(cudaEventRecord(pl.ev[&up - &pl.units[0]], s));
     if (!grad) {
-      if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s)); else CK(launch_tuned_jk(w, u.nblocks, s));
+      if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s));
+      else if (u.kernel == 3) CK(launch_tile_jk_class(w, u.t_nblocks, s));
+      else CK(launch_tuned_jk(w, u.nblocks, s));
     } else {
       if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s)); else CK(launch_tuned_grad(w, u.g_nblocks, s));
     }
@@ -430,6 +525,8 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
     init_pair_class(b, pc->ga, pc->gb, *np);
     for (int i : idx) { np->sa.push_back(pc->sa[i]); np->sb.push_back(pc->sb[i]); np->wgt.push_back(pc->wgt[i]); np->Q.push_back(pc->Q[i]); }
     CKI(upload_pair_class(b, *np, s));
+    np->hrr_loss = hrr_loss_of(b, *np);
+    CKI(make_grouped(b, *np, s));
     pairs_kept += np->npair;
     pl.pcs.push_back(std::move(np));
   }
@@ -699,13 +796,14 @@ int eri_plan_class_stats(const eri_plan_t* cplan, eri_class_stat_t* out, int max
     eri_class_stat_t& c = out[k++];
     c.la = P.la; c.lb = P.lb; c.lc = R.la; c.ld = R.lb; c.ka = P.Ka; c.kb = P.Kb; c.kc = R.Ka; c.kd = R.Kb;
     c.nroots = (P.la + P.lb + R.la + R.lb) / 2 + 1; c.kernel = u.kernel; c.quartets = u.quartets;
+    c.slots = plan->is_list ? u.quartets : u.kernel == 3 ? u.t_slots : (long long)u.nblocks * u.BI * u.BJ;
     c.canonical_flops = u.flops; c.last_ms = u.last_ms; c.last_ms_grad = u.last_ms_grad;
   }
   return k;
 }
 int eri_plan_set_timing(eri_plan_t* plan, int on) { if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan"); plan->timing = on; return ERI_OK; }
 int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode) {
-  if (!plan || mode < 0 || mode > 1) return fail(ERI_ERR_BAD_ARG, "bad kernel mode");
+  if (!plan || mode < 0 || mode > 2) return fail(ERI_ERR_BAD_ARG, "bad kernel mode");
   plan->kernel_mode = mode;
   for (auto& u : plan->units) CKI(select_kernels(*plan, *u, nullptr));
   return ERI_OK;

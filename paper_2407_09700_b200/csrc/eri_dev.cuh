@@ -109,6 +109,11 @@ struct Work {
   double* gK;
   int nao;
   int shard, nshard; // this process runs the blocks b = blockIdx.x * nshard + shard (eri_plan_set_shard)
+  // tile family (tile_kernel.cuh): bra/ket are GROUPED pair sets (chunks of 32 slots sharing the first shell, q < 0 marks
+  // a padding slot); row r = the BI bra slots starting at row_slot[r], its blocks = the first row_off[r+1]-row_off[r] ket
+  // chunks; a quartet is evaluated iff q_i * q_j >= thr (and j <= i when bra set == ket set) -- the same set as dense mode.
+  const int* row_slot;
+  double thr;
 };
 
 __device__ __forceinline__ void atomic_add(double* p, double v) { atomicAdd(p, v); }

@@ -14,7 +14,10 @@ cudaError_t launch_generic_store(const Work& w, double* out, const long long* of
 cudaError_t launch_generic_grad(const Work& w, int nblocks_dense, cudaStream_t s);
 
 // tuned kernels: a launcher per l-class; returns false in `*handled` when the class has no tuned kernel.
-struct TunedInfo { int kind; int BI, BJ; };   // kind: 1 register-unrolled, 2 cooperative; tile shape for dense mode
+struct TunedInfo { int kind; int BI, BJ; int TQ; };   // kind: 1 register-unrolled, 2 cooperative, 3 tile; tile shape for dense mode
+// tile family (kind 3, dense mode only): threads per quartet TQ and bra rows per block BI of the class, false if not served
+bool tile_jk_info(int la, int lb, int lc, int ld, TunedInfo* info);
+cudaError_t launch_tile_jk_class(const Work& w, int nblocks_dense, cudaStream_t s);
 bool tuned_jk_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info);
 cudaError_t launch_tuned_jk(const Work& w, int nblocks_dense, cudaStream_t s);
 bool tuned_grad_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info);

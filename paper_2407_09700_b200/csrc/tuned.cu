@@ -2,6 +2,7 @@
 #include "launch.h"
 #include "reg_classes.h"
 #include "coop_classes.h"
+#include "tile_classes.h"
 
 namespace eri {
 
@@ -51,6 +52,31 @@ cudaError_t launch_tuned_jk(const Work& w, int nblocks, cudaStream_t s) {
   if (launch_reg_group2(key, w, nblocks, s, &err)) return err;
   if (launch_reg_group3(key, w, nblocks, s, &err)) return err;
 #define TRY(g) if (launch_coop_group##g(key, w, nblocks, s, &err)) return err;
+  TRY(0) TRY(1) TRY(2) TRY(3) TRY(4) TRY(5) TRY(6) TRY(7)
+#undef TRY
+  return cudaErrorNotSupported;
+}
+
+// ---- tile family (dense mode only) ----
+#define DECL(g) bool launch_tile_group##g(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+DECL(0) DECL(1) DECL(2) DECL(3) DECL(4) DECL(5) DECL(6) DECL(7)
+#undef DECL
+static_assert(TILE_NGROUPS == 8, "tuned.cu lists eight tile groups");
+#define TILE_ALL(X) TILE_GROUP0(X) TILE_GROUP1(X) TILE_GROUP2(X) TILE_GROUP3(X) TILE_GROUP4(X) TILE_GROUP5(X) TILE_GROUP6(X) TILE_GROUP7(X)
+
+bool tile_jk_info(int la, int lb, int lc, int ld, TunedInfo* info) {
+  switch (la * 1000 + lb * 100 + lc * 10 + ld) {
+#define X(a, b, c, d, tq, bi) case a * 1000 + b * 100 + c * 10 + d: info->kind = 3; info->TQ = tq; info->BI = bi; info->BJ = 32; return true;
+    TILE_ALL(X)
+#undef X
+    default: return false;
+  }
+}
+
+cudaError_t launch_tile_jk_class(const Work& w, int nblocks, cudaStream_t s) {
+  const int key = w.bra.la * 1000 + w.bra.lb * 100 + w.ket.la * 10 + w.ket.lb;
+  cudaError_t err = cudaErrorNotSupported;
+#define TRY(g) if (launch_tile_group##g(key, w, nblocks, s, &err)) return err;
   TRY(0) TRY(1) TRY(2) TRY(3) TRY(4) TRY(5) TRY(6) TRY(7)
 #undef TRY
   return cudaErrorNotSupported;

@@ -56,6 +56,12 @@ def test_tuned_kernels_are_selected(eri):
     kinds = {}
     for c in plan.class_stats():
         kinds.setdefault((c["la"], c["lb"], c["lc"], c["ld"]), set()).add(c["kernel"])
+    assert all(k.issubset({1, 2, 3}) for k in kinds.values()), kinds
+    assert kinds[(3, 3, 3, 3)] == {2}
+    plan.set_kernel_mode(2)   # register and cooperative families only
+    kinds = {}
+    for c in plan.class_stats():
+        kinds.setdefault((c["la"], c["lb"], c["lc"], c["ld"]), set()).add(c["kernel"])
     assert kinds[(0, 0, 0, 0)] == {1} and kinds[(2, 1, 1, 0)] == {1}
     assert kinds[(2, 1, 2, 1)] == {2} and kinds[(2, 2, 2, 1)] == {2}
     plan.set_kernel_mode(1)
