@@ -292,7 +292,9 @@ int schwarz_of_class(PairClass& pc, cudaStream_t s) {
 }
 
 // ---- work units -----------------------------------------------------------------------------------------------
-constexpr double TILE_MIN_FILL = 0.3;   // tile family only where at least this fraction of the swept lanes has work
+// tile family only where at least TILE_MIN_FILL of the swept lanes has work and the bra chunks hold enough rows to amortise
+// the block-end reduction (measured on cfg3)
+constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3;
 constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
 
 struct Unit {
@@ -417,7 +419,7 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
         slots += 32 * n;
       }
     }
-    if (slots > 0 && (double)u.quartets / (double)slots >= TILE_MIN_FILL) {
+    if (slots > 0 && (double)u.quartets / (double)slots >= TILE_MIN_FILL && gb.fill >= TILE_MIN_BRA_FILL) {
       if (getenv("ERI_DEBUG_UNITS")) fprintf(stderr, "UNIT %d %d %d %d %d %d %d %d eff %.3f brafill %.3f ketfill %.3f\n", P.la, P.lb, R.la, R.lb, P.Ka, P.Kb, R.Ka, R.Kb,
                                            (double)u.quartets / (double)slots, gb.fill, gk.fill);
       u.kernel = 3; u.tBI = ti.BI; u.t_slots = slots;

@@ -179,6 +179,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
   double* __restrict__ Jm = w.J; double* __restrict__ Km = w.K;
   int a0 = -1;                         // first Cartesian AO of shell a owned by this thread
 
+#pragma unroll 1
   for (int y = gq; y < TILE_ROWS; y += BI) {
     const int i = i_first + y;
     const double qi = bp.q[i];
