@@ -173,6 +173,7 @@ struct PairClass {
   std::unique_ptr<PairClass> grouped;
   std::vector<double> chunk_q;     // grouped only: largest Schwarz factor of each chunk (chunks are sorted by it, descending)
   double fill = 0.0;               // grouped only: valid slots / slots
+  double hrr_loss_grad = 1.0;      // the same with lb + 1 quanta (gradient kernels raise the second shell too)
   double hrr_loss = 1.0;           // max over primitive pairs of ((alpha_a + alpha_b) / alpha_a)^lb, see DESIGN.md "HRR direction"
   PairSet view() const {
     PairSet v; v.prim = prim.p; v.geom = geom.p; v.aexp = aexp.p; v.q = q.p; v.ao = ao.p; v.atom = atom.p;
@@ -218,8 +219,8 @@ int upload_pair_class(const Basis& b, PairClass& pc, cudaStream_t s) {
 }
 
 // digits lost by the horizontal transfer when the 2-D integrals are built on the FIRST centre: |AB| / |PB| = p / alpha_a per quantum
-double hrr_loss_of(const Basis& b, const PairClass& pc) {
-  if (pc.lb == 0) return 1.0;
+double hrr_loss_of(const Basis& b, const PairClass& pc, int extra) {
+  if (pc.lb + extra == 0) return 1.0;
   double worst = 1.0;
   for (size_t i = 0; i < pc.sa.size(); ++i) {
     const eri_shell_t& A = b.sh[pc.sa[i]]; const eri_shell_t& B = b.sh[pc.sb[i]];
@@ -227,7 +228,7 @@ double hrr_loss_of(const Basis& b, const PairClass& pc) {
     for (int ka = 0; ka < A.nprim; ++ka)
       for (int kb = 0; kb < B.nprim; ++kb) {
         const double ea = b.pr[A.prim_off + ka].exp, eb = b.pr[B.prim_off + kb].exp;
-        worst = std::max(worst, std::pow((ea + eb) / ea, pc.lb));
+        worst = std::max(worst, std::pow((ea + eb) / ea, pc.lb + extra));
       }
   }
   return worst;
@@ -294,7 +295,8 @@ int schwarz_of_class(PairClass& pc, cudaStream_t s) {
 // ---- work units -----------------------------------------------------------------------------------------------
 // tile family only where at least TILE_MIN_FILL of the swept lanes has work and the bra chunks hold enough rows to amortise
 // the block-end reduction (measured on cfg3)
-constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3;
+constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3, TILE_MIN_FILL_COOP = 0.25, TILE_MIN_FILL_GRAD = 0.1;
+constexpr double HRR_LOSS_MAX_GRAD = 1.0e5;   // gradient tolerance is 1e-8 Ha/Bohr absolute
 constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
 
 struct Unit {
@@ -321,7 +323,7 @@ struct eri_plan {
   Basis basis;
   bool is_list = false, want_grad = false;
   double thr = 0.0;
-  int kernel_mode = 0, timing = 0, shard = 0, nshard = 1;
+  int kernel_mode = 0, timing = 0, shard = 0, nshard = 1, serial = 0;
   std::vector<std::unique_ptr<PairClass>> pcs;
   std::vector<std::unique_ptr<Unit>> units;
   Dev<int> sh_l, sh_sph, sh_cart, sph2sh, cart2sh;
@@ -330,7 +332,16 @@ struct eri_plan {
   eri_stats_t stats{};
   std::vector<cudaEvent_t> ev;   // timing mode: ev[k] before unit k, ev[n] after the last one (no host sync in between)
   bool ev_pending = false, ev_grad = false;
-  ~eri_plan() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
+  // concurrent mode (default outside timing mode): the units are independent (they merge by atomic add), so they
+  // are dealt over a small pool of streams, heaviest first, forked from and joined to the caller's stream with events
+  std::vector<cudaStream_t> pool; std::vector<cudaEvent_t> pool_ev; cudaEvent_t fork_ev = nullptr;
+  std::vector<int> order, order_grad;   // unit indices by decreasing cost
+  ~eri_plan() {
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : pool_ev) cudaEventDestroy(e);
+    for (cudaStream_t st : pool) cudaStreamDestroy(st);
+    if (fork_ev) cudaEventDestroy(fork_ev);
+  }
 };
 
 namespace eri {
@@ -395,40 +406,43 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
   const bool canonical = P.la >= P.lb && R.la >= R.lb && (P.la > R.la || (P.la == R.la && P.lb >= R.lb));
   if (pl.kernel_mode != 1 && canonical && tuned_jk_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel = ti.kind; u.BI = ti.BI; u.BJ = ti.BJ; }
   // tile family: dense mode, and only where building the 2-D integrals on the first centre of every pair is safe
-  if (pl.kernel_mode == 0 && canonical && !pl.is_list && P.grouped && R.grouped && P.hrr_loss <= HRR_LOSS_MAX && R.hrr_loss <= HRR_LOSS_MAX &&
-      tile_jk_info(P.la, P.lb, R.la, R.lb, &ti)) {
+  u.kernel_grad = 0; u.gBI = GENERIC_GRAD_BI; u.gBJ = GENERIC_GRAD_BJ;
+  if (pl.kernel_mode == 0 && canonical && !pl.is_list && P.grouped && R.grouped) {
     const PairClass& gb = *P.grouped; const PairClass& gk = *R.grouped;
-    const int nbc = (int)gb.chunk_q.size(), nkc = (int)gk.chunk_q.size();
-    std::vector<int> slot, off{0};
-    long long slots = 0;
-    std::vector<double> rq(32);
-    for (int cb = 0; cb < nbc; ++cb) {   // one block per (bra chunk, ket chunk of the prefix that passes Schwarz)
-      const double qb = gb.chunk_q[cb];
-      int lo = 0, hi = nkc;
-      if (pl.thr > 0.0) { while (lo < hi) { const int mid = (lo + hi) / 2; if (qb * gk.chunk_q[mid] >= pl.thr) lo = mid + 1; else hi = mid; } }
-      else lo = nkc;
-      if (u.same) lo = std::min(lo, cb + 1);
-      if (lo == 0) continue;
-      slot.push_back(32 * cb); off.push_back(off.back() + lo);
-      // lane slots actually swept = rows with work x 32 (the kernel skips the other rows)
-      for (int y = 0; y < 32; ++y) rq[y] = gb.Q[32 * cb + y];
-      std::sort(rq.begin(), rq.end(), std::greater<double>());
-      for (int ck = 0; ck < lo; ++ck) {
-        int n = 0;
-        while (n < 32 && rq[n] >= 0.0 && rq[n] * gk.chunk_q[ck] >= pl.thr) ++n;
-        slots += 32 * n;
+    if (u.t_nblocks == 0) {   // blocks of the tile decomposition (independent of the class kernel): once per unit
+      const int nbc = (int)gb.chunk_q.size(), nkc = (int)gk.chunk_q.size();
+      std::vector<int> slot, off{0};
+      long long slots = 0;
+      std::vector<double> rq(32);
+      for (int cb = 0; cb < nbc; ++cb) {   // one block per (bra chunk, ket chunk of the prefix that passes Schwarz)
+        const double qb = gb.chunk_q[cb];
+        int lo = 0, hi = nkc;
+        if (pl.thr > 0.0) { while (lo < hi) { const int mid = (lo + hi) / 2; if (qb * gk.chunk_q[mid] >= pl.thr) lo = mid + 1; else hi = mid; } }
+        else lo = nkc;
+        if (u.same) lo = std::min(lo, cb + 1);
+        if (lo == 0) continue;
+        slot.push_back(32 * cb); off.push_back(off.back() + lo);
+        // lane slots actually swept = rows with work x 32 (the kernel skips the other rows)
+        for (int y = 0; y < 32; ++y) rq[y] = gb.Q[32 * cb + y];
+        for (int ck = 0; ck < lo; ++ck) {
+          int nr = 0;
+          while (nr < 32 && rq[nr] >= 0.0 && rq[nr] * gk.chunk_q[ck] >= pl.thr) ++nr;
+          slots += 32 * nr;
+        }
       }
-    }
-    if (slots > 0 && (double)u.quartets / (double)slots >= TILE_MIN_FILL && gb.fill >= TILE_MIN_BRA_FILL) {
-      if (getenv("ERI_DEBUG_UNITS")) fprintf(stderr, "UNIT %d %d %d %d %d %d %d %d eff %.3f brafill %.3f ketfill %.3f\n", P.la, P.lb, R.la, R.lb, P.Ka, P.Kb, R.Ka, R.Kb,
-                                           (double)u.quartets / (double)slots, gb.fill, gk.fill);
-      u.kernel = 3; u.tBI = ti.BI; u.t_slots = slots;
-      u.t_nrows = (int)slot.size(); u.t_nblocks = off.back();
+      u.t_slots = slots; u.t_nrows = (int)slot.size(); u.t_nblocks = off.back();
       CK(u.t_row_slot.upload(slot, s)); CK(u.t_row_off.upload(off, s));
     }
+    const double fill = u.t_slots > 0 ? (double)u.quartets / (double)u.t_slots : 0.0;
+    if (P.hrr_loss <= HRR_LOSS_MAX && R.hrr_loss <= HRR_LOSS_MAX && tile_jk_info(P.la, P.lb, R.la, R.lb, &ti)) {
+      // the register family (kind 1) is hard to beat on sparsely filled tiles; the cooperative family (kind 2) is not
+      const bool take = u.kernel == 1 ? (fill >= TILE_MIN_FILL && gb.fill >= TILE_MIN_BRA_FILL) : fill >= (ti.TQ >= 5 ? TILE_MIN_FILL : TILE_MIN_FILL_COOP);
+      if (take) { u.kernel = 3; u.tBI = ti.BI; }
+    }
+    // gradient: one more quantum is transferred (lb + 1, ld + 1 is not raised), so the loss bound is one power higher
+    if (pl.want_grad && fill >= TILE_MIN_FILL_GRAD && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
+        tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = 3; u.gBI = ti.BI; }
   }
-  u.kernel_grad = 0; u.gBI = GENERIC_GRAD_BI; u.gBJ = GENERIC_GRAD_BJ;
-  if (pl.kernel_mode == 0 && canonical && tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = ti.kind; u.gBI = ti.BI; u.gBJ = ti.BJ; }
   if (!pl.is_list) {
     std::vector<int> ro;
     make_rows(u.h_count, u.BI, u.BJ, ro);
@@ -451,7 +465,7 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
   w.row_off = grad ? u.g_row_off.p : u.row_off.p;
   w.nrows = grad ? u.g_nrows : u.nrows;
   w.thr = pl.thr;
-  if (!grad && u.kernel == 3) {
+  if (grad ? u.kernel_grad == 3 : u.kernel == 3) {
     w.bra = pl.pcs[u.P]->grouped->view(); w.ket = pl.pcs[u.R]->grouped->view();
     w.row_off = u.t_row_off.p; w.row_slot = u.t_row_slot.p; w.nrows = u.t_nrows;
   }
@@ -462,22 +476,54 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
   return w;
 }
 
+constexpr int POOL_STREAMS = 8;
+
+int launch_unit(eri_plan& pl, Unit& u, bool grad, double* gJ, double* gK, cudaStream_t s) {
+  Work w = make_work(pl, u, grad);
+  w.gJ = gJ; w.gK = gK;
+  if (!grad) {
+    if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s));
+    else if (u.kernel == 3) CK(launch_tile_jk_class(w, u.t_nblocks, s));
+    else CK(launch_tuned_jk(w, u.nblocks, s));
+  } else {
+    if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s)); else CK(launch_tuned_grad(w, u.t_nblocks, s));
+  }
+  return ERI_OK;
+}
+
 int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
-  if (pl.timing) while (pl.ev.size() < pl.units.size() + 1) { cudaEvent_t e; CK(cudaEventCreate(&e)); pl.ev.push_back(e); }
-  for (auto& up : pl.units) {
-    Unit& u = *up;
-    Work w = make_work(pl, u, grad);
-    w.gJ = gJ; w.gK = gK;
-    if (pl.timing) CK(cudaEventRecord(pl.ev[&up - &pl.units[0]], s));
-    if (!grad) {
-      if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s));
-      else if (u.kernel == 3) CK(launch_tile_jk_class(w, u.t_nblocks, s));
-      else CK(launch_tuned_jk(w, u.nblocks, s));
-    } else {
-      if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s)); else CK(launch_tuned_grad(w, u.g_nblocks, s));
+  const int nu = (int)pl.units.size();
+  if (pl.timing) {   // serial, one event between launches: per-unit device times
+    while ((int)pl.ev.size() < nu + 1) { cudaEvent_t e; CK(cudaEventCreate(&e)); pl.ev.push_back(e); }
+    for (int k = 0; k < nu; ++k) {
+      CK(cudaEventRecord(pl.ev[k], s));
+      CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
+    }
+    CK(cudaEventRecord(pl.ev[nu], s)); pl.ev_pending = true; pl.ev_grad = grad;
+    return ERI_OK;
+  }
+  if (nu < 2 || pl.serial) {
+    for (int k = 0; k < nu; ++k) CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
+    return ERI_OK;
+  }
+  if (pl.pool.empty()) {
+    CK(cudaEventCreateWithFlags(&pl.fork_ev, cudaEventDisableTiming));
+    for (int k = 0; k < POOL_STREAMS; ++k) {
+      cudaStream_t st; CK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)); pl.pool.push_back(st);
+      cudaEvent_t e; CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); pl.pool_ev.push_back(e);
     }
   }
-  if (pl.timing) { CK(cudaEventRecord(pl.ev[pl.units.size()], s)); pl.ev_pending = true; pl.ev_grad = grad; }
+  std::vector<int>& order = grad ? pl.order_grad : pl.order;
+  if ((int)order.size() != nu) {
+    order.resize(nu);
+    for (int k = 0; k < nu; ++k) order[k] = k;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
+      return (grad ? pl.units[x]->flops_grad : pl.units[x]->flops) > (grad ? pl.units[y]->flops_grad : pl.units[y]->flops); });
+  }
+  CK(cudaEventRecord(pl.fork_ev, s));
+  for (cudaStream_t st : pl.pool) CK(cudaStreamWaitEvent(st, pl.fork_ev, 0));
+  for (int k = 0; k < nu; ++k) CKI(launch_unit(pl, *pl.units[order[k]], grad, gJ, gK, pl.pool[k % POOL_STREAMS]));
+  for (int k = 0; k < POOL_STREAMS; ++k) { CK(cudaEventRecord(pl.pool_ev[k], pl.pool[k])); CK(cudaStreamWaitEvent(s, pl.pool_ev[k], 0)); }
   return ERI_OK;
 }
 
@@ -527,7 +573,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
     init_pair_class(b, pc->ga, pc->gb, *np);
     for (int i : idx) { np->sa.push_back(pc->sa[i]); np->sb.push_back(pc->sb[i]); np->wgt.push_back(pc->wgt[i]); np->Q.push_back(pc->Q[i]); }
     CKI(upload_pair_class(b, *np, s));
-    np->hrr_loss = hrr_loss_of(b, *np);
+    np->hrr_loss = hrr_loss_of(b, *np, 0); np->hrr_loss_grad = hrr_loss_of(b, *np, 1);
     CKI(make_grouped(b, *np, s));
     pairs_kept += np->npair;
     pl.pcs.push_back(std::move(np));
