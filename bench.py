@@ -260,7 +260,7 @@ def main():
                 "class_kernels_share_of_step": kern_ms / ms if ms else None,
                 "top_class": None if top is None else {"l": [top["la"], top["lb"], top["lc"], top["ld"]], "k": [top["ka"], top["kb"], top["kc"], top["kd"]],
                                                        "ms": top[key], "quartets": top["quartets"],
-                                                       "tflops": (top["canonical_flops"] / (top[key] * 1e-3) / 1e12) if (top[key] > 0 and kind != "grad") else None}}
+                                                       "tflops": ((top["canonical_flops_grad"] if kind == "grad" else top["canonical_flops"]) / (top[key] * 1e-3) / 1e12) if top[key] > 0 else None}}
     cb = None
     if not args.no_cpu_baseline and world == 1:
         cb = cpu_baseline(kind, basis, D, quartets)
@@ -278,9 +278,9 @@ def main():
             for u, c in enumerate(classes):
                 c["unit"] = u
             for c in sorted(classes, key=lambda c: -c[key]):
-                fl = c["canonical_flops"] if kind != "grad" else 0.0
+                fl = c["canonical_flops"] if kind != "grad" else c["canonical_flops_grad"]
                 tf = fl / (c[key] * 1e-3) / 1e12 if c[key] > 0 else 0.0
-                f.write(f"{c['la']} {c['lb']} {c['lc']} {c['ld']} {c['ka']} {c['kb']} {c['kc']} {c['kd']} {c['nroots']} {c['kernel']} "
+                f.write(f"{c['la']} {c['lb']} {c['lc']} {c['ld']} {c['ka']} {c['kb']} {c['kc']} {c['kd']} {c['nroots']} {c['kernel_grad'] if kind == 'grad' else c['kernel']} "
                         f"{c['quartets']} {c[key]:.4f} {fl / 1e9:.3f} {tf:.3f} {100 * tf / fp64_peak:.2f} {c['unit']} {c['slots']}\n")
     print(json.dumps(line))
     if dist is not None:

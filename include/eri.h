@@ -75,6 +75,9 @@ typedef struct {
   double canonical_flops;     /* per call                                                      */
   float last_ms;              /* device time of the unit's last launch; needs eri_plan_set_timing(plan,1)      */
   float last_ms_grad;
+  int32_t kernel_grad;        /* gradient kernel of the unit: 0 generic, 3 tile                  */
+  int32_t reserved_;
+  double canonical_flops_grad;
 } eri_class_stat_t;
 
 /* ---- one-shot calls (north-star signatures).  shells/prims/coords HOST; D, J, K, grad_* DEVICE. ---------------- */

@@ -477,6 +477,7 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
 }
 
 constexpr int POOL_STREAMS = 8;
+constexpr long long POOL_BIG_BLOCKS = 4 * 148;   // at least four blocks per SM: the launch fills the GPU
 
 int launch_unit(eri_plan& pl, Unit& u, bool grad, double* gJ, double* gK, cudaStream_t s) {
   Work w = make_work(pl, u, grad);
@@ -522,7 +523,15 @@ int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
   }
   CK(cudaEventRecord(pl.fork_ev, s));
   for (cudaStream_t st : pl.pool) CK(cudaStreamWaitEvent(st, pl.fork_ev, 0));
-  for (int k = 0; k < nu; ++k) CKI(launch_unit(pl, *pl.units[order[k]], grad, gJ, gK, pl.pool[k % POOL_STREAMS]));
+  // launches that fill the GPU by themselves stay on the caller's stream, one after the other (they only disturb each other
+  // when they overlap); the many small ones (deeply contracted pair sets with few pairs) share the pool and fill the gaps
+  int small = 0;
+  for (int k = 0; k < nu; ++k) {
+    Unit& u = *pl.units[order[k]];
+    const long long blocks = grad ? (u.kernel_grad == 3 ? u.t_nblocks : u.g_nblocks) : (u.kernel == 3 ? u.t_nblocks : u.nblocks);
+    const bool big = blocks / pl.nshard >= POOL_BIG_BLOCKS;
+    CKI(launch_unit(pl, u, grad, gJ, gK, big ? s : pl.pool[small++ % POOL_STREAMS]));
+  }
   for (int k = 0; k < POOL_STREAMS; ++k) { CK(cudaEventRecord(pl.pool_ev[k], pl.pool[k])); CK(cudaStreamWaitEvent(s, pl.pool_ev[k], 0)); }
   return ERI_OK;
 }
@@ -846,6 +855,7 @@ int eri_plan_class_stats(const eri_plan_t* cplan, eri_class_stat_t* out, int max
     c.nroots = (P.la + P.lb + R.la + R.lb) / 2 + 1; c.kernel = u.kernel; c.quartets = u.quartets;
     c.slots = plan->is_list ? u.quartets : u.kernel == 3 ? u.t_slots : (long long)u.nblocks * u.BI * u.BJ;
     c.canonical_flops = u.flops; c.last_ms = u.last_ms; c.last_ms_grad = u.last_ms_grad;
+    c.kernel_grad = u.kernel_grad; c.canonical_flops_grad = u.flops_grad;
   }
   return k;
 }
