@@ -171,7 +171,7 @@ struct PairClass {
   // tile family: the same pairs in chunks of 32 slots that share the first shell (padding slots have Q = -1);
   // chunks are ordered by decreasing largest Schwarz factor, which is the factor of the chunk's first slot
   std::unique_ptr<PairClass> grouped;
-  std::vector<double> chunk_q;     // grouped only: largest Schwarz factor of each chunk (chunks are sorted by it, descending)
+  std::vector<double> half_q;      // grouped only: largest Schwarz factor of each half-chunk of 16 slots (sorted by it, descending; -1: padding)
   double fill = 0.0;               // grouped only: valid slots / slots
   double hrr_loss_grad = 1.0;      // the same with lb + 1 quanta (gradient kernels raise the second shell too)
   double hrr_loss = 1.0;           // max over primitive pairs of ((alpha_a + alpha_b) / alpha_a)^lb, see DESIGN.md "HRR direction"
@@ -237,27 +237,31 @@ double hrr_loss_of(const Basis& b, const PairClass& pc, int extra) {
 void init_pair_class(const Basis& b, int ga, int gb, PairClass& pc);
 
 // grouped twin of a Schwarz-sorted pair set (tile family): every first shell's partner list (sorted by decreasing Q) is cut
-// into chunks of 32 slots, the chunks are sorted by their head's Q; padding slots have Q = -1.
+// into HALVES of 16 slots, the halves are sorted by their head's Q and two consecutive halves make a chunk of 32 slots
+// (= the lanes of a warp when the set is the ket; a bra tile is one half); padding slots have Q = -1.
+constexpr int HALF = 16;
 int make_grouped(const Basis& b, PairClass& pc, cudaStream_t s) {
   auto gp = std::make_unique<PairClass>();
   init_pair_class(b, pc.ga, pc.gb, *gp);
   std::map<int, std::vector<int>> by_first;
   for (int i = 0; i < pc.npair; ++i) by_first[pc.sa[i]].push_back(i);   // pc is sorted by decreasing Q, so is every group
-  struct Chunk { double q; const std::vector<int>* idx; int begin, n; };
-  std::vector<Chunk> chunks;
+  struct Half { double q; const std::vector<int>* idx; int begin, n; };
+  std::vector<Half> halves;
   for (auto& kv : by_first)
-    for (int st = 0; st < (int)kv.second.size(); st += 32)
-      chunks.push_back(Chunk{pc.Q[kv.second[st]], &kv.second, st, std::min(32, (int)kv.second.size() - st)});
-  std::stable_sort(chunks.begin(), chunks.end(), [](const Chunk& x, const Chunk& y) { return x.q > y.q; });
-  for (const Chunk& c : chunks) {
-    gp->chunk_q.push_back(c.q);
-    for (int t = 0; t < 32; ++t) {
-      const int src = (*c.idx)[c.begin + (t < c.n ? t : 0)];   // padding repeats the chunk's first pair (valid addresses)
+    for (int st = 0; st < (int)kv.second.size(); st += HALF)
+      halves.push_back(Half{pc.Q[kv.second[st]], &kv.second, st, std::min(HALF, (int)kv.second.size() - st)});
+  std::stable_sort(halves.begin(), halves.end(), [](const Half& x, const Half& y) { return x.q > y.q; });
+  const size_t nvalid = halves.size();
+  if (halves.size() % 2) halves.push_back(Half{-1.0, halves.back().idx, halves.back().begin, 0});   // an all-padding half
+  for (const Half& c : halves) {
+    gp->half_q.push_back(c.q);
+    for (int t = 0; t < HALF; ++t) {
+      const int src = (*c.idx)[c.begin + (t < c.n ? t : 0)];   // padding repeats a pair of the half (valid addresses, same first shell)
       gp->sa.push_back(pc.sa[src]); gp->sb.push_back(pc.sb[src]); gp->wgt.push_back(pc.wgt[src]);
       gp->Q.push_back(t < c.n ? pc.Q[src] : -1.0);
     }
   }
-  gp->fill = chunks.empty() ? 0.0 : (double)pc.npair / (32.0 * chunks.size());
+  gp->fill = nvalid == 0 ? 0.0 : (double)pc.npair / ((double)HALF * nvalid);
   CKI(upload_pair_class(b, *gp, s));
   pc.grouped = std::move(gp);
   return ERI_OK;
@@ -410,23 +414,22 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
   if (pl.kernel_mode == 0 && canonical && !pl.is_list && P.grouped && R.grouped) {
     const PairClass& gb = *P.grouped; const PairClass& gk = *R.grouped;
     if (u.t_nblocks == 0) {   // blocks of the tile decomposition (independent of the class kernel): once per unit
-      const int nbc = (int)gb.chunk_q.size(), nkc = (int)gk.chunk_q.size();
+      const int nbh = (int)gb.half_q.size(), nkc = (int)gk.half_q.size() / 2;
       std::vector<int> slot, off{0};
       long long slots = 0;
-      std::vector<double> rq(32);
-      for (int cb = 0; cb < nbc; ++cb) {   // one block per (bra chunk, ket chunk of the prefix that passes Schwarz)
-        const double qb = gb.chunk_q[cb];
-        int lo = 0, hi = nkc;
-        if (pl.thr > 0.0) { while (lo < hi) { const int mid = (lo + hi) / 2; if (qb * gk.chunk_q[mid] >= pl.thr) lo = mid + 1; else hi = mid; } }
+      for (int hb = 0; hb < nbh; ++hb) {   // one block per (bra half, ket chunk of the prefix that passes Schwarz)
+        const double qb = gb.half_q[hb];
+        if (qb < 0.0) continue;
+        int lo = 0, hi = nkc;   // the first half of a ket chunk carries the chunk's largest factor
+        if (pl.thr > 0.0) { while (lo < hi) { const int mid = (lo + hi) / 2; if (qb * gk.half_q[2 * mid] >= pl.thr) lo = mid + 1; else hi = mid; } }
         else lo = nkc;
-        if (u.same) lo = std::min(lo, cb + 1);
+        if (u.same) lo = std::min(lo, hb / 2 + 1);
         if (lo == 0) continue;
-        slot.push_back(32 * cb); off.push_back(off.back() + lo);
-        // lane slots actually swept = rows with work x 32 (the kernel skips the other rows)
-        for (int y = 0; y < 32; ++y) rq[y] = gb.Q[32 * cb + y];
+        slot.push_back(HALF * hb); off.push_back(off.back() + lo);
+        // lane slots actually swept = rows with work x 32 (the kernel skips the other rows; rows are sorted within the half)
         for (int ck = 0; ck < lo; ++ck) {
           int nr = 0;
-          while (nr < 32 && rq[nr] >= 0.0 && rq[nr] * gk.chunk_q[ck] >= pl.thr) ++nr;
+          while (nr < HALF && gb.Q[HALF * hb + nr] >= 0.0 && gb.Q[HALF * hb + nr] * gk.half_q[2 * ck] >= pl.thr) ++nr;
           slots += 32 * nr;
         }
       }

@@ -5,9 +5,9 @@
 // Cartesian element contributes  dI/dR . (PJ, PK)  straight into 18 per-thread scalars (reading R10/R11:
 // PJ = 4 f D_ab D_cd, PK = 2 f (D_ab' ...) = 2 f (D_ac D_bd + D_ad D_bc)) -- there is no per-element accumulator, so the
 // footprint does not grow with Pi nc(l).  The six density blocks of a quartet are staged in shared memory: the three
-// that are the same for all lanes of a row (D_ab, D_ac, D_bc) once per warp, the three that depend on the ket's second
-// shell (D_cd, D_ad, D_bd) in a column per lane.  The 18 scalars are summed over the lanes through the warp's
-// shared-memory transpose and leave as 18 FP64 atomics per ROW (the paper: 12 atomics per quartet);
+// that do not depend on the ket's second shell (D_ab once per warp; D_ac, D_bc once per ket half), the three that do
+// (D_cd, D_ad, D_bd) in a column per lane.  The 18 scalars are summed over the lanes through the warp's
+// shared-memory transpose and leave as at most 36 FP64 atomics per ROW (one sum per ket half) (the paper: 12 atomics per quartet);
 // the centre-D part is kept per lane over the rows and leaves once per block.
 #pragma once
 #include "tile_kernel.cuh"
@@ -19,7 +19,7 @@ struct TileGradTraits {
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
   static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
   static constexpr int G2 = (LA + 2) * (LB + 2) * (LC + 2) * (LD + 1);          // raised on A, B, C
-  static constexpr int NUNI = NA * NB + NA * NC + NB * NC;                        // D_ab, D_ac, D_bc: per warp
+  static constexpr int NUNI = NA * NB + 2 * (NA * NC + NB * NC);                 // D_ab per warp; D_ac, D_bc per ket half
   static constexpr int NLANE = NC * ND + NA * ND + NB * ND;                       // D_cd, D_ad, D_bd: per lane
   static constexpr int STAGE = 32 * 33;
   static constexpr int PERWARP = STAGE + NUNI + 32 * NLANE;
@@ -106,7 +106,8 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
   double* stage = smem + gq * Tr::PERWARP;
   double* uni = stage + Tr::STAGE;                 // [D_ab | D_ac | D_bc], the same for all lanes
   double* mine = uni + Tr::NUNI + x;               // column of this lane, stride 32: [D_cd | D_ad | D_bd]
-  double* Dab_s = uni; double* Dac_s = uni + NA * NB; double* Dbc_s = Dac_s + NA * NC;
+  const int half = x >> 4;                         // ket half of this lane: its own shell c
+  double* Dab_s = uni; double* Dac_s = uni + NA * NB + half * (NA * NC + NB * NC); double* Dbc_s = Dac_s + NA * NC;
   double* Dcd_s = mine; double* Dad_s = mine + 32 * NC * ND; double* Dbd_s = Dad_s + 32 * NA * ND;
 
   const int j = j_first + x;
@@ -140,8 +141,8 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
     // ---- density blocks of this row ----
     __syncwarp();
     for (int e = x; e < NA * NB; e += 32) Dab_s[e] = D[(long)(a0 + e / NB) * n + b0 + e % NB];
-    for (int e = x; e < NA * NC; e += 32) Dac_s[e] = D[(long)(a0 + e / NC) * n + c0 + e % NC];
-    for (int e = x; e < NB * NC; e += 32) Dbc_s[e] = D[(long)(b0 + e / NC) * n + c0 + e % NC];
+    for (int e = x & 15; e < NA * NC; e += 16) Dac_s[e] = D[(long)(a0 + e / NC) * n + c0 + e % NC];   // each half stages its own c
+    for (int e = x & 15; e < NB * NC; e += 16) Dbc_s[e] = D[(long)(b0 + e / NC) * n + c0 + e % NC];
 #pragma unroll
     for (int a = 0; a < NA; ++a)
 #pragma unroll
@@ -276,10 +277,10 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
     }
     // centres A, B (fixed for the row) and C (shared by the lanes): sum over the lanes, 18 atomics per row
     const int2 at_ab = bp.atom[i];
-    const int atC = kp.atom[j_first].x;
-    warp_reduce_values<18>(acc, stage, x, [&](int v, double sum) {
+    const int atC_lo = kp.atom[j_first].x, atC_hi = kp.atom[j_first + 16].x;   // the two ket halves have their own shell c
+    warp_reduce_values<18, true>(acc, stage, x, [&](int v, int half, double sum) {
       const int jk = v / 9, ce = (v % 9) / 3, ax = v % 3;
-      const int at = ce == 0 ? at_ab.x : ce == 1 ? at_ab.y : atC;
+      const int at = ce == 0 ? at_ab.x : ce == 1 ? at_ab.y : half ? atC_hi : atC_lo;
       atomic_add((jk ? w.gK : w.gJ) + 3 * at + ax, sum);
     });
   }

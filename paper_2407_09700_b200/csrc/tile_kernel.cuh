@@ -3,9 +3,10 @@
 // quartet in registers and then issues six FP64 atomics PER ELEMENT.  On sm_100a a
 // scattered FP64 reduction costs more SM time than the arithmetic of a low-l quartet, so this family keeps the
 // register-resident evaluation and changes everything around it:
-//   * pairs are laid out in CHUNKS of 32 slots that share their first shell and are sorted by decreasing Schwarz factor
-//     (api.cu, "grouped pair sets"); a block is (one bra chunk) x (one ket chunk): all rows share shell a, all lanes
-//     share shell c.  A warp takes one bra row at a time (lane = ket slot) and skips the rows that Schwarz rules out;
+//   * pairs are laid out in HALF-CHUNKS of 16 slots that share their first shell and are sorted by decreasing Schwarz
+//     factor (api.cu, "grouped pair sets"); a block is (one bra half: 16 rows, one shell a) x (one ket chunk: two halves
+//     = the 32 lanes of a warp, one shell c per half).  A warp takes one bra row at a time (lane = ket slot) and skips
+//     the rows that Schwarz rules out;
 //   * a quartet is evaluated by TQ threads that sit in TQ different warps (same lane): each owns NA/TQ Cartesian
 //     components of shell a and recomputes the (cheap) 2-D integrals, so that its accumulators fit in registers and
 //     no warp ever diverges;
@@ -21,7 +22,7 @@
 
 namespace eri {
 
-constexpr int TILE_ROWS = 32;   // bra slots per chunk = rows of a block's tile
+constexpr int TILE_ROWS = 16;   // bra slots per half-chunk = rows of a block's tile (they share the first shell a)
 
 // 2-D integrals of one axis and one root in registers: G[((i*(LB+1)+j)*(LC+1)+k)*(LD+1)+l] (reading R5).
 template <int LA, int LB, int LC, int LD>
@@ -113,9 +114,11 @@ __device__ __forceinline__ void tile_product(double* __restrict__ g, const doubl
   }
 }
 
-// Sum of NV per-lane values over the 32 lanes of a warp: lanes stage their values in the warp's private region
-// stage[32][33] (value-row major, 32 values per batch), lane l adds up value-row l and hands the sum to emit(v, sum).
-template <int NV, class F>
+// Sum of NV per-lane values over the lanes of a warp: lanes stage their values in the warp's private region
+// stage[32][33] (value-row major, 32 values per batch) and lane l adds up value-row l.  HALVES = false: one sum over the
+// 32 lanes, emit(v, 0, sum).  HALVES = true: lanes 0-15 and 16-31 belong to two half-chunks of the ket set (different
+// first shells c), so the two halves are summed separately, emit(v, half, sum).
+template <int NV, bool HALVES, class F>
 __device__ __forceinline__ void warp_reduce_values(const double* __restrict__ v, double* __restrict__ stage, int lane, F emit) {
 #pragma unroll
   for (int b0 = 0; b0 < NV; b0 += 32) {
@@ -128,9 +131,15 @@ __device__ __forceinline__ void warp_reduce_values(const double* __restrict__ v,
       const double* row = stage + lane * 33;
       double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
 #pragma unroll
-      for (int k = 0; k < 32; k += 4) { s0 += row[k]; s1 += row[k + 1]; s2 += row[k + 2]; s3 += row[k + 3]; }
-      const double sum = (s0 + s1) + (s2 + s3);
-      if (sum != 0.0) emit(b0 + lane, sum);
+      for (int k = 0; k < 16; k += 2) { s0 += row[k]; s1 += row[k + 1]; s2 += row[16 + k]; s3 += row[17 + k]; }
+      if (HALVES) {
+        const double lo = s0 + s1, hi = s2 + s3;
+        if (lo != 0.0) emit(b0 + lane, 0, lo);
+        if (hi != 0.0) emit(b0 + lane, 1, hi);
+      } else {
+        const double sum = (s0 + s1) + (s2 + s3);
+        if (sum != 0.0) emit(b0 + lane, 0, sum);
+      }
     }
   }
 }
@@ -174,6 +183,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
   for (int o = 16; o > 0; o >>= 1) qk_max = fmax(qk_max, __shfl_xor_sync(0xffffffffu, qk_max, o));
   const int2 cd0 = kp.ao[j];
   const int c0 = cd0.x, d0 = cd0.y;
+  const int c0_lo = __shfl_sync(0xffffffffu, c0, 0), c0_hi = __shfl_sync(0xffffffffu, c0, 16);   // shell c of the two ket halves
   const int n = w.nao;
   const double* __restrict__ D = w.D;
   double* __restrict__ Jm = w.J; double* __restrict__ Km = w.K;
@@ -257,7 +267,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
         for (int cd = 0; cd < NCD; ++cd) sacc = fma(g[ab * NCD + cd], Dcd[cd], sacc);
         v[ab] = sacc;
       }
-      warp_reduce_values<NABT>(v, stage, x, [&](int vi, double sum) { atomic_add(Jm + (long)(a0 + vi / NB) * n + b0 + vi % NB, sum); });
+      warp_reduce_values<NABT, false>(v, stage, x, [&](int vi, int, double sum) { atomic_add(Jm + (long)(a0 + vi / NB) * n + b0 + vi % NB, sum); });
     }
     {  // J_cd += sum_ab g D_ab ; kept per lane over the rows.  D_ab is the same for all lanes (broadcast loads)
       double v[NCD];
@@ -274,7 +284,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
 #pragma unroll
       for (int cd = 0; cd < NCD; ++cd) keep[cd * NT] += v[cd];
     }
-    {  // K_ac += sum_bd g D_bd ; summed over the lanes (they share c)
+    {  // K_ac += sum_bd g D_bd ; summed over the lanes of each ket half (they share c)
       double Dbd[NB * ND];
 #pragma unroll
       for (int b = 0; b < NB; ++b)
@@ -292,7 +302,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
             for (int d = 0; d < ND; ++d) sacc = fma(g[((a * NB + b) * NC + c) * ND + d], Dbd[b * ND + d], sacc);
           v[a * NC + c] = sacc;
         }
-      warp_reduce_values<NAT * NC>(v, stage, x, [&](int vi, double sum) { atomic_add(Km + (long)(a0 + vi / NC) * n + c0 + vi % NC, sum); });
+      warp_reduce_values<NAT * NC, true>(v, stage, x, [&](int vi, int half, double sum) { atomic_add(Km + (long)(a0 + vi / NC) * n + (half ? c0_hi : c0_lo) + vi % NC, sum); });
     }
     {  // K_ad += sum_bc g D_bc ; kept per lane over the rows (they share a).  D_bc is the same for all lanes
       double v[NAT * ND];
@@ -311,7 +321,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
 #pragma unroll
       for (int e = 0; e < NAT * ND; ++e) keep[(NCD + e) * NT] += v[e];
     }
-    {  // K_bc += sum_ad g D_ad ; summed over the lanes
+    {  // K_bc += sum_ad g D_ad ; summed over the lanes of each ket half
       double Dad[NAT * ND];
 #pragma unroll
       for (int a = 0; a < NAT; ++a)
@@ -329,7 +339,7 @@ __global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
             for (int d = 0; d < ND; ++d) sacc = fma(g[((a * NB + b) * NC + c) * ND + d], Dad[a * ND + d], sacc);
           v[b * NC + c] = sacc;
         }
-      warp_reduce_values<NB * NC>(v, stage, x, [&](int vi, double sum) { atomic_add(Km + (long)(b0 + vi / NC) * n + c0 + vi % NC, sum); });
+      warp_reduce_values<NB * NC, true>(v, stage, x, [&](int vi, int half, double sum) { atomic_add(Km + (long)(b0 + vi / NC) * n + (half ? c0_hi : c0_lo) + vi % NC, sum); });
     }
     if (active) {  // K_bd += sum_ac g D_ac ; private to the quartet
       double v[NB * ND];
