@@ -446,6 +446,10 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
     if (pl.want_grad && fill >= TILE_MIN_FILL_GRAD && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
         tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = 3; u.gBI = ti.BI; }
   }
+  // cooperative gradient kernel for what the tile gradient kernel does not serve (it chooses the build centre itself)
+  if (pl.kernel_mode != 1 && pl.want_grad && canonical && !pl.is_list && u.kernel_grad == 0 && coop_grad_info(P.la, P.lb, R.la, R.lb, &ti)) {
+    u.kernel_grad = 2; u.gBI = ti.BI; u.gBJ = ti.BJ;
+  }
   if (!pl.is_list) {
     std::vector<int> ro;
     make_rows(u.h_count, u.BI, u.BJ, ro);
@@ -490,7 +494,9 @@ int launch_unit(eri_plan& pl, Unit& u, bool grad, double* gJ, double* gK, cudaSt
     else if (u.kernel == 3) CK(launch_tile_jk_class(w, u.t_nblocks, s));
     else CK(launch_tuned_jk(w, u.nblocks, s));
   } else {
-    if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s)); else CK(launch_tuned_grad(w, u.t_nblocks, s));
+    if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s));
+    else if (u.kernel_grad == 2) CK(launch_coop_grad_class(w, u.g_nblocks, s));
+    else CK(launch_tuned_grad(w, u.t_nblocks, s));
   }
   return ERI_OK;
 }

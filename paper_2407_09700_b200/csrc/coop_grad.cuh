@@ -1,0 +1,242 @@
+// coop_grad.cuh -- cooperative family, J/K gradient kernel (Algorithm 4; Eq. 11-15)
+// for the classes whose unrolled thread-per-quartet body (tile_grad.cuh) does not fit the register file.
+// One WARP per shell quartet, as in coop_kernel.cuh:
+//   phase 1  lane (root r, axis x) builds the 2-D integrals with the indices of centres A, B, C raised by one
+//            (centre D follows from translational invariance) on the numerically safe centres and stores
+//            them to the warp's shared-memory slab S[axis][root][i][j][k][l];
+//   phase 2  lane `ab` owns a Cartesian bra component pair; for every ket component pair and root it forms
+//            F[I] = 2 alpha I(+1) - n I(-1) (Eq. 11) on the three centres and three axes and adds
+//            dI/dR . (PJ, PK) (reading R10/R11) into 18 per-lane scalars -- no per-element accumulator;
+//   phase 3  the 18 scalars are summed over the lanes through the (dead) slab: centres A and B leave per quartet,
+//            centres C and D are kept over the bra pairs of the warp's task and leave once per task.
+// A task is one ket pair and a run of CH consecutive bra pairs of the Schwarz-sorted tile row (dense mode).
+#pragma once
+#include "coop_kernel.cuh"
+#include "tile_kernel.cuh"   // warp_reduce_values
+
+namespace eri {
+
+constexpr int CGRAD_CH = 16;      // bra pairs per task
+
+template <int LA, int LB, int LC, int LD, int WARPS>   // WARPS = ket pairs per block (gen_class_lists.py sizes it for 200 KB of shared memory)
+struct CoopGradTraits {
+  static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+  static constexpr int NAB = NA * NB, NCD = NC * ND;
+  static constexpr int PASSES = (NAB + 31) / 32;
+  static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
+  static constexpr int SCD = (LC + 2) * (LD + 1), G2 = (LA + 2) * (LB + 2) * SCD;   // raised on A, B, C
+  static constexpr int SLAB2D = 3 * N * G2;
+  static constexpr int SLAB = (SLAB2D > 32 * 33 ? SLAB2D : 32 * 33) + NCD;          // + staged D_cd
+  static constexpr size_t SMEM = sizeof(double) * SLAB * WARPS;
+  static_assert(SMEM <= 227 * 1024, "slab does not fit");
+  static_assert(3 * N <= 32, "one lane per (root, axis)");
+};
+
+template <int LA, int LB, int LC, int LD, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS) coop_grad_kernel(Work w) {
+  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS>;
+  constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
+  constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2;
+  constexpr int SL = 1, SK = LD + 1, SJ = SCD, SI = (LB + 2) * SCD;   // strides of (i, j, k, l) in the slab
+  extern __shared__ double smem[];
+  const int lane = threadIdx.x, wy = threadIdx.y;
+  double* S = smem + (size_t)wy * Tr::SLAB;
+  double* sDcd = S + (Tr::SLAB - NCD);
+
+  const PairSet& bp = w.bra; const PairSet& kp = w.ket;
+  const int blk = blockIdx.x * w.nshard + w.shard;
+  if (blk >= w.row_off[w.nrows]) return;
+  const int r = find_row(w.row_off, w.nrows, blk);
+  const int j = (blk - w.row_off[r]) * WARPS + wy;
+  const int i_begin = r * CGRAD_CH, i_end = min(i_begin + CGRAD_CH, bp.npair);
+  if (j >= kp.npair) return;
+  const int n = w.nao;
+  const double* __restrict__ D = w.D;
+
+  // ---- per-task ket data ----
+  double C[3], CD[3];
+#pragma unroll
+  for (int x = 0; x < 3; ++x) { C[x] = kp.geom[x * kp.stride + j]; CD[x] = kp.geom[(3 + x) * kp.stride + j]; }
+  const double wket = kp.geom[6 * kp.stride + j];
+  const int c0 = kp.ao[j].x, d0 = kp.ao[j].y;
+  for (int cd = lane; cd < NCD; cd += 32) sDcd[cd] = D[(long)(c0 + cd / ND) * n + d0 + cd % ND];
+  __syncwarp();
+
+  const int my_root = lane / 3, my_axis = lane - 3 * my_root;
+  const bool fill_lane = lane < 3 * N;
+  double keepC = 0.0, keepD = 0.0;   // lane v < 18: centre-C sum of value v (if v is a C value) and its share of centre D, over the task
+
+  for (int i = i_begin; i < i_end; ++i) {
+    if (j >= w.ket_count[i]) continue;     // warp-uniform
+    double f = bp.geom[6 * bp.stride + i] * wket;
+    if (w.same && i == j) f *= 0.5;
+    double A[3], AB[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) { A[x] = bp.geom[x * bp.stride + i]; AB[x] = bp.geom[(3 + x) * bp.stride + i]; }
+    const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
+
+    double acc[18];   // [J: A xyz, B xyz, C xyz | K: same]
+#pragma unroll
+    for (int e = 0; e < 18; ++e) acc[e] = 0.0;
+
+    for (int kb = 0; kb < bp.npp; ++kb) {
+      const double p = bp.prim[(kb * 5 + 0) * bp.stride + i];
+      const double P[3] = {bp.prim[(kb * 5 + 1) * bp.stride + i], bp.prim[(kb * 5 + 2) * bp.stride + i], bp.prim[(kb * 5 + 3) * bp.stride + i]};
+      const double Kab = bp.prim[(kb * 5 + 4) * bp.stride + i];
+      const double ea2 = 2.0 * bp.aexp[(kb * 2 + 0) * bp.stride + i], eb2 = 2.0 * bp.aexp[(kb * 2 + 1) * bp.stride + i];
+      bool swb;   // build on B when P is nearer to B (the raised index of B is always transferred)
+      {
+        double da = 0.0, db = 0.0;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { const double pa = P[x] - A[x], pb = pa + AB[x]; da += pa * pa; db += pb * pb; }
+        swb = db < da;
+      }
+      for (int kk = 0; kk < kp.npp; ++kk) {
+        const double q = kp.prim[(kk * 5 + 0) * kp.stride + j];
+        const double Q[3] = {kp.prim[(kk * 5 + 1) * kp.stride + j], kp.prim[(kk * 5 + 2) * kp.stride + j], kp.prim[(kk * 5 + 3) * kp.stride + j]};
+        const double Kcd = kp.prim[(kk * 5 + 4) * kp.stride + j];
+        const double ec2 = 2.0 * kp.aexp[(kk * 2 + 0) * kp.stride + j];
+        bool swk = false;
+        if (LD > 0) {
+          double dc = 0.0, dd = 0.0;
+#pragma unroll
+          for (int x = 0; x < 3; ++x) { const double qc = Q[x] - C[x], qd = qc + CD[x]; dc += qc * qc; dd += qd * qd; }
+          swk = dd < dc;
+        }
+        const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+        const double PQ[3] = {P[0] - Q[0], P[1] - Q[1], P[2] - Q[2]};
+        const double xx = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
+        // ---- phase 1 ----
+        __syncwarp();
+        if (fill_lane) {
+          double u, wt;
+          rys_root_one<N>(xx, w.rys, my_root, u, wt);
+          const double t2 = u * rpq;
+          const double b00 = 0.5 * t2, b10 = (1.0 - q * t2) * 0.5 / p, b01 = (1.0 - p * t2) * 0.5 / q;
+          const int ax = my_axis;
+          const double pa = (ax == 0 ? P[0] - A[0] : ax == 1 ? P[1] - A[1] : P[2] - A[2]);
+          const double qc = (ax == 0 ? Q[0] - C[0] : ax == 1 ? Q[1] - C[1] : Q[2] - C[2]);
+          const double pqx = (ax == 0 ? PQ[0] : ax == 1 ? PQ[1] : PQ[2]);
+          const double abx = (ax == 0 ? AB[0] : ax == 1 ? AB[1] : AB[2]);
+          const double cdx = (ax == 0 ? CD[0] : ax == 1 ? CD[1] : CD[2]);
+          const double c00 = pa + (swb ? abx : 0.0) - q * t2 * pqx;
+          const double c00p = qc + (swk ? cdx : 0.0) + p * t2 * pqx;
+          const double init = ax == 2 ? f * Kab * Kcd * sqrt(rpq) * wt : 1.0;
+          double* dst = S + (ax * N + my_root) * G2;
+          if (!swb) {
+            if (!swk) fill_2d_smem<LA + 1, LB + 1, LC + 1, LD>(dst, SI, SJ, SK, SL, init, c00, c00p, b10, b01, b00, abx, cdx);
+            else if constexpr (LD > 0) fill_2d_smem<LA + 1, LB + 1, LD, LC + 1>(dst, SI, SJ, SL, SK, init, c00, c00p, b10, b01, b00, abx, -cdx);
+          } else {
+            if (!swk) fill_2d_smem<LB + 1, LA + 1, LC + 1, LD>(dst, SJ, SI, SK, SL, init, c00, c00p, b10, b01, b00, -abx, cdx);
+            else if constexpr (LD > 0) fill_2d_smem<LB + 1, LA + 1, LD, LC + 1>(dst, SJ, SI, SL, SK, init, c00, c00p, b10, b01, b00, -abx, -cdx);
+          }
+        }
+        __syncwarp();
+        // ---- phase 2 ----
+#pragma unroll
+        for (int ps = 0; ps < PASSES; ++ps) {
+          int ab = lane + 32 * ps;
+          const bool own = ab < NAB;
+          if (!own) ab = NAB - 1;
+          const int ia = ab / NB, ib = ab - ia * NB;
+          int ax, ay, az, bx, by, bz;
+          cart_powers(LA, ia, ax, ay, az); cart_powers(LB, ib, bx, by, bz);
+          const long ra = (long)(a0 + ia) * n, rb = (long)(b0 + ib) * n;
+          const double dab = own ? D[ra + b0 + ib] : 0.0;
+          double Dac[NC], Dbc[NC], Dad[ND], Dbd[ND];
+#pragma unroll
+          for (int c = 0; c < NC; ++c) { Dac[c] = own ? D[ra + c0 + c] : 0.0; Dbc[c] = own ? D[rb + c0 + c] : 0.0; }
+#pragma unroll
+          for (int d = 0; d < ND; ++d) { Dad[d] = D[ra + d0 + d]; Dbd[d] = D[rb + d0 + d]; }
+          const int ox = (ax * SI + bx * SJ), oy = (ay * SI + by * SJ) + N * G2, oz = (az * SI + bz * SJ) + 2 * N * G2;
+          const double fax = (double)ax, fay = (double)ay, faz = (double)az, fbx = (double)bx, fby = (double)by, fbz = (double)bz;
+#pragma unroll 1
+          for (int rt = 0; rt < N; ++rt) {
+            const double* X = S + ox + rt * G2;
+            const double* Y = S + oy + rt * G2;
+            const double* Z = S + oz + rt * G2;
+            int c = 0;
+#pragma unroll
+            for (int cx = LC; cx >= 0; --cx)
+#pragma unroll
+            for (int cy = LC - cx; cy >= 0; --cy) {
+              const int cz = LC - cx - cy;
+              int d = 0;
+#pragma unroll
+              for (int dx = LD; dx >= 0; --dx)
+#pragma unroll
+              for (int dy = LD - dx; dy >= 0; --dy) {
+                const int dz = LD - dx - dy;
+                const int ex = cx * SK + dx, ey = cy * SK + dy, ez = cz * SK + dz;
+                const double vx = X[ex], vy = Y[ey], vz = Z[ez];
+                const double oyz = vy * vz, oxz = vx * vz, oxy = vx * vy;
+                // lowered terms vanish with their integer factor; the slab has no index -1, so guard the address
+                const double dAx = fma(ea2, X[ex + SI], -fax * X[ax > 0 ? ex - SI : ex]);
+                const double dAy = fma(ea2, Y[ey + SI], -fay * Y[ay > 0 ? ey - SI : ey]);
+                const double dAz = fma(ea2, Z[ez + SI], -faz * Z[az > 0 ? ez - SI : ez]);
+                const double dBx = fma(eb2, X[ex + SJ], -fbx * X[bx > 0 ? ex - SJ : ex]);
+                const double dBy = fma(eb2, Y[ey + SJ], -fby * Y[by > 0 ? ey - SJ : ey]);
+                const double dBz = fma(eb2, Z[ez + SJ], -fbz * Z[bz > 0 ? ez - SJ : ez]);
+                const double dCx = cx > 0 ? fma(ec2, X[ex + SK], -cx * X[ex - SK]) : ec2 * X[ex + SK];
+                const double dCy = cy > 0 ? fma(ec2, Y[ey + SK], -cy * Y[ey - SK]) : ec2 * Y[ey + SK];
+                const double dCz = cz > 0 ? fma(ec2, Z[ez + SK], -cz * Z[ez - SK]) : ec2 * Z[ez + SK];
+                const double pj = dab * sDcd[c * ND + d];
+                const double pk = fma(Dac[c], Dbd[d], Dad[d] * Dbc[c]);
+                const double jx = pj * oyz, jy = pj * oxz, jz = pj * oxy;
+                const double kx = pk * oyz, ky = pk * oxz, kz = pk * oxy;
+                acc[0] = fma(dAx, jx, acc[0]); acc[1] = fma(dAy, jy, acc[1]); acc[2] = fma(dAz, jz, acc[2]);
+                acc[3] = fma(dBx, jx, acc[3]); acc[4] = fma(dBy, jy, acc[4]); acc[5] = fma(dBz, jz, acc[5]);
+                acc[6] = fma(dCx, jx, acc[6]); acc[7] = fma(dCy, jy, acc[7]); acc[8] = fma(dCz, jz, acc[8]);
+                acc[9] = fma(dAx, kx, acc[9]); acc[10] = fma(dAy, ky, acc[10]); acc[11] = fma(dAz, kz, acc[11]);
+                acc[12] = fma(dBx, kx, acc[12]); acc[13] = fma(dBy, ky, acc[13]); acc[14] = fma(dBz, kz, acc[14]);
+                acc[15] = fma(dCx, kx, acc[15]); acc[16] = fma(dCy, ky, acc[16]); acc[17] = fma(dCz, kz, acc[17]);
+                ++d;
+              }
+              ++c;
+            }
+          }
+        }
+      }
+    }
+
+    // ---- phase 3: PJ = 4 f ..., PK = 2 f ... (f is in the prefactor); sum over the lanes through the dead slab ----
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { acc[e] *= 4.0; acc[9 + e] *= 2.0; }
+    const int2 at_ab = bp.atom[i];
+    // lane v = jk*9 + centre*3 + axis receives the sum of value v: centres A, B leave now; the lane keeps its C sum and
+    // its share of centre D = -(A + B + C) until the task ends
+    warp_reduce_values<18, false>(acc, S, lane, [&](int v, int, double sum) {
+      const int jk = v / 9, ce = (v % 9) / 3, ax = v % 3;
+      if (ce < 2) atomic_add((jk ? w.gK : w.gJ) + 3 * (ce == 0 ? at_ab.x : at_ab.y) + ax, sum);
+      else keepC += sum;
+      keepD -= sum;
+    });
+    __syncwarp();
+  }
+
+  // ---- task end ----
+  if (lane < 18) {
+    const int jk = lane / 9, ax = lane % 3;
+    const int2 at_cd = kp.atom[j];
+    double* gout = jk ? w.gK : w.gJ;
+    if (keepC != 0.0) atomic_add(gout + 3 * at_cd.x + ax, keepC);
+    if (keepD != 0.0) atomic_add(gout + 3 * at_cd.y + ax, keepD);
+  }
+}
+
+template <int LA, int LB, int LC, int LD, int WARPS>
+cudaError_t launch_coop_grad(const Work& w, int nblocks_dense, cudaStream_t s) {
+  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS>;
+  const int grid = (nblocks_dense + w.nshard - 1) / w.nshard;
+  if (grid <= 0) return cudaSuccess;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(coop_grad_kernel<LA, LB, LC, LD, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  coop_grad_kernel<LA, LB, LC, LD, WARPS><<<grid, dim3(32, WARPS), Tr::SMEM, s>>>(w);
+  return cudaGetLastError();
+}
+
+}  // namespace eri

@@ -22,6 +22,9 @@ bool tuned_jk_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, Tun
 cudaError_t launch_tuned_jk(const Work& w, int nblocks_dense, cudaStream_t s);
 bool tuned_grad_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info);
 cudaError_t launch_tuned_grad(const Work& w, int nblocks_dense, cudaStream_t s);
+// cooperative gradient kernel (kind 2, dense mode): info->BI x info->BJ = bra pairs per task x ket pairs per block
+bool coop_grad_info(int la, int lb, int lc, int ld, TunedInfo* info);
+cudaError_t launch_coop_grad_class(const Work& w, int nblocks_dense, cudaStream_t s);
 
 // transform.cu
 cudaError_t upload_c2s(const double* tables /*host, concatenated ns(l) x nc(l), l = 0..4*/);

@@ -4,6 +4,7 @@
 #include "coop_classes.h"
 #include "tile_classes.h"
 #include "tile_grad_classes.h"
+#include "coop_grad_classes.h"
 
 namespace eri {
 
@@ -89,6 +90,31 @@ DECL(0) DECL(1) DECL(2) DECL(3) DECL(4) DECL(5) DECL(6) DECL(7)
 #undef DECL
 static_assert(TGRAD_NGROUPS == 8, "tuned.cu lists eight tile gradient groups");
 #define TGRAD_ALL(X) TGRAD_GROUP0(X) TGRAD_GROUP1(X) TGRAD_GROUP2(X) TGRAD_GROUP3(X) TGRAD_GROUP4(X) TGRAD_GROUP5(X) TGRAD_GROUP6(X) TGRAD_GROUP7(X)
+
+#define DECL(g) bool launch_cgrad_group##g(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+DECL(0) DECL(1) DECL(2) DECL(3) DECL(4) DECL(5) DECL(6) DECL(7)
+#undef DECL
+static_assert(CGRAD_NGROUPS == 8, "tuned.cu lists eight cooperative gradient groups");
+#define CGRAD_ALL(X) CGRAD_GROUP0(X) CGRAD_GROUP1(X) CGRAD_GROUP2(X) CGRAD_GROUP3(X) CGRAD_GROUP4(X) CGRAD_GROUP5(X) CGRAD_GROUP6(X) CGRAD_GROUP7(X)
+
+// cooperative gradient kernel (kind 2): Schwarz-sorted pair sets, task = 16 bra pairs x 1 ket pair, `warps` ket pairs per block
+bool coop_grad_info(int la, int lb, int lc, int ld, TunedInfo* info) {
+  switch (la * 1000 + lb * 100 + lc * 10 + ld) {
+#define X(a, b, c, d, wp) case a * 1000 + b * 100 + c * 10 + d: info->kind = 2; info->TQ = 1; info->BI = 16; info->BJ = wp; return true;
+    CGRAD_ALL(X)
+#undef X
+    default: return false;
+  }
+}
+
+cudaError_t launch_coop_grad_class(const Work& w, int nblocks, cudaStream_t s) {
+  const int key = w.bra.la * 1000 + w.bra.lb * 100 + w.ket.la * 10 + w.ket.lb;
+  cudaError_t err = cudaErrorNotSupported;
+#define TRY(g) if (launch_cgrad_group##g(key, w, nblocks, s, &err)) return err;
+  TRY(0) TRY(1) TRY(2) TRY(3) TRY(4) TRY(5) TRY(6) TRY(7)
+#undef TRY
+  return cudaErrorNotSupported;
+}
 
 bool tuned_grad_info(int la, int lb, int lc, int ld, int, int, TunedInfo* info) {
   switch (la * 1000 + lb * 100 + lc * 10 + ld) {
