@@ -24,7 +24,7 @@ struct CoopGradTraits {
   static constexpr int NAB = NA * NB, NCD = NC * ND;
   static constexpr int PASSES = (NAB + 31) / 32;
   static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
-  static constexpr int SCD = (LC + 2) * (LD + 1), G2 = (LA + 2) * (LB + 2) * SCD;   // raised on A, B, C
+  static constexpr int SCD = ((LC + 2) * (LD + 1)) | 1, G2 = ((LA + 2) * (LB + 2) * SCD) | 1;   // raised on A, B, C; odd strides: no bank conflicts
   static constexpr int SLAB2D = 3 * N * G2;
   static constexpr int SLAB = (SLAB2D > 32 * 33 ? SLAB2D : 32 * 33) + NCD;          // + staged D_cd
   static constexpr size_t SMEM = sizeof(double) * SLAB * WARPS;

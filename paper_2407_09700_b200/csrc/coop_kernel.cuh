@@ -113,7 +113,9 @@ struct CoopTraits {
   static constexpr int NAB = NA * NB, NCD = NC * ND;
   static constexpr int PASSES = (NAB + T - 1) / T;
   static constexpr int N = nroots_of(LA + LB + LC + LD);
-  static constexpr int SCD = (LC + 1) * (LD + 1), G2 = (LA + 1) * (LB + 1) * SCD;
+  // strides of the slab: SCD = one (i,j) row, G2 = one (axis, root) block; both padded to odd so that lanes that differ in
+  // (i,j) (phase 2 loads) or in (axis, root) (phase 1 stores) fall into different shared-memory banks
+  static constexpr int SCD = ((LC + 1) * (LD + 1)) | 1, G2 = ((LA + 1) * (LB + 1) * SCD) | 1;
   static constexpr int SLAB2D = 3 * N * G2;
   static constexpr int KROW = (2 * (NC + ND)) | 1;           // per (a,b): Kac[NC] Kad[ND] Kbc[NC] Kbd[ND]; odd stride: no bank conflicts
   static constexpr int SLABK = PASSES * T * KROW;
