@@ -120,25 +120,45 @@ __device__ __forceinline__ void tile_product(double* __restrict__ g, const doubl
 // first shells c), so the two halves are summed separately, emit(v, half, sum).
 template <int NV, bool HALVES, class F>
 __device__ __forceinline__ void warp_reduce_values(const double* __restrict__ v, double* __restrict__ stage, int lane, F emit) {
-#pragma unroll
-  for (int b0 = 0; b0 < NV; b0 += 32) {
-    const int nb = NV - b0 < 32 ? NV - b0 : 32;
+  if constexpr (NV <= 16) {
+    // few values: all 32 lanes work.  ROWS value-rows x LPR lanes per row; a lane adds ROWS staged elements of its row
+    // (interleaved, within its ket half if HALVES), then the LPR (LPR/2) lanes of a row (half) finish with shuffles.
+    constexpr int ROWS = NV <= 1 ? 1 : NV <= 2 ? 2 : NV <= 4 ? 4 : NV <= 8 ? 8 : 16;
+    constexpr int LPR = 32 / ROWS, GRP = HALVES ? LPR / 2 : LPR;   // lanes that share one sum
     __syncwarp();
 #pragma unroll
-    for (int i = 0; i < 32; ++i) if (i < nb) stage[i * 33 + lane] = v[b0 + i];
+    for (int i = 0; i < NV; ++i) stage[i * 33 + lane] = v[i];
     __syncwarp();
-    if (lane < nb) {
-      const double* row = stage + lane * 33;
-      double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    const int row = lane / LPR, sl = lane - row * LPR;
+    const int half = HALVES ? sl / GRP : 0, t = sl - half * GRP;
+    const double* src = stage + row * 33 + 16 * half + t;
+    double sum = 0.0;
 #pragma unroll
-      for (int k = 0; k < 16; k += 2) { s0 += row[k]; s1 += row[k + 1]; s2 += row[16 + k]; s3 += row[17 + k]; }
-      if (HALVES) {
-        const double lo = s0 + s1, hi = s2 + s3;
-        if (lo != 0.0) emit(b0 + lane, 0, lo);
-        if (hi != 0.0) emit(b0 + lane, 1, hi);
-      } else {
-        const double sum = (s0 + s1) + (s2 + s3);
-        if (sum != 0.0) emit(b0 + lane, 0, sum);
+    for (int m = 0; m < ROWS; ++m) sum += src[m * GRP];
+#pragma unroll
+    for (int o = GRP / 2; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if (t == 0 && row < NV && sum != 0.0) emit(row, half, sum);
+  } else {
+#pragma unroll
+    for (int b0 = 0; b0 < NV; b0 += 32) {
+      const int nb = NV - b0 < 32 ? NV - b0 : 32;
+      __syncwarp();
+#pragma unroll
+      for (int i = 0; i < 32; ++i) if (i < nb) stage[i * 33 + lane] = v[b0 + i];
+      __syncwarp();
+      if (lane < nb) {
+        const double* row = stage + lane * 33;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+        for (int k = 0; k < 16; k += 2) { s0 += row[k]; s1 += row[k + 1]; s2 += row[16 + k]; s3 += row[17 + k]; }
+        if (HALVES) {
+          const double lo = s0 + s1, hi = s2 + s3;
+          if (lo != 0.0) emit(b0 + lane, 0, lo);
+          if (hi != 0.0) emit(b0 + lane, 1, hi);
+        } else {
+          const double sum = (s0 + s1) + (s2 + s3);
+          if (sum != 0.0) emit(b0 + lane, 0, sum);
+        }
       }
     }
   }
