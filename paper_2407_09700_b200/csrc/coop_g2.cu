@@ -5,7 +5,7 @@
 namespace eri {
 bool launch_coop_group2(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err) {
   switch (key) {
-#define X(a, b, c, d, tw) case a * 1000 + b * 100 + c * 10 + d: *err = launch_coop_jk<a, b, c, d, tw>(w, nblocks, s); return true;
+#define X(a, b, c, d, tw, nch) case a * 1000 + b * 100 + c * 10 + d: *err = launch_coop_jk<a, b, c, d, tw, nch>(w, nblocks, s); return true;
     COOP_GROUP2(X)
 #undef X
     default: return false;

@@ -106,10 +106,14 @@ __device__ __forceinline__ void group_sync(int tw, int id) {
   else asm volatile("bar.sync %0, %1;" ::"r"(id + 1), "r"(32 * tw) : "memory");
 }
 
-template <int LA, int LB, int LC, int LD, int TW>
+// NCH > 1: the Cartesian components of shell c are split into NCH chunks and blockIdx.y selects the chunk, so that the
+// accumulators per lane, PASSES * (nc(lc) / NCH) * nc(ld), stay in registers for the heaviest classes ((gf|ff) ... (gg|gg));
+// the 2-D integrals are then rebuilt once per chunk (cheap next to the products of such classes).
+template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
 struct CoopTraits {
   static constexpr int T = 32 * TW, GROUPS = COOP_WARPS / TW;
-  static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+  static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC) / NCH, ND = ncart(LD);   // NC: components of c per chunk
+  static_assert(ncart(LC) % NCH == 0, "NCH must divide the number of Cartesian components of shell c");
   static constexpr int NAB = NA * NB, NCD = NC * ND;
   static constexpr int PASSES = (NAB + T - 1) / T;
   static constexpr int N = nroots_of(LA + LB + LC + LD);
@@ -123,9 +127,9 @@ struct CoopTraits {
   static constexpr size_t SMEM = sizeof(double) * SLAB * GROUPS;
 };
 
-template <int LA, int LB, int LC, int LD, int TW>
+template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
 __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
-  using Tr = CoopTraits<LA, LB, LC, LD, TW>;
+  using Tr = CoopTraits<LA, LB, LC, LD, TW, NCH>;
   constexpr int T = Tr::T, GROUPS = Tr::GROUPS;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
   constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2;
@@ -157,9 +161,19 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
 #pragma unroll
   for (int x = 0; x < 3; ++x) { C[x] = kp.geom[x * kp.stride + j]; CD[x] = kp.geom[(3 + x) * kp.stride + j]; }
   const double wket = kp.geom[6 * kp.stride + j];
-  const int c0 = kp.ao[j].x, d0 = kp.ao[j].y;
+  const int c_lo = NCH > 1 ? (int)blockIdx.y * NC : 0;   // first component of this block's chunk of shell c
+  const int c0 = kp.ao[j].x + c_lo, d0 = kp.ao[j].y;     // everything below addresses D, J, K through c0: chunk-local c
   for (int cd = lane; cd < NCD; cd += T) sDcd[cd] = D[(long)(c0 + cd / ND) * n + d0 + cd % ND];
   group_sync(TW, wy);
+  int ocx[NCH > 1 ? NC : 1], ocy[NCH > 1 ? NC : 1], ocz[NCH > 1 ? NC : 1];   // slab offsets of the chunk's components (NCH > 1)
+  if (NCH > 1) {
+#pragma unroll
+    for (int cl = 0; cl < NC; ++cl) {
+      int px, py, pz;
+      cart_powers(LC, c_lo + cl, px, py, pz);
+      ocx[cl] = px * (LD + 1); ocy[cl] = py * (LD + 1); ocz[cl] = pz * (LD + 1);
+    }
+  }
 
   // ---- per-lane roles ---------------------------------------------------------------------------------------------
   // phase 1: lane -> (root, axis)
@@ -261,6 +275,20 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
             const double* X = S + offx[ps] + r * G2;
             const double* Y = S + offy[ps] + r * G2;
             const double* Z = S + offz[ps] + r * G2;
+            if constexpr (NCH > 1) {
+#pragma unroll
+              for (int cl = 0; cl < NC; ++cl) {
+                int d = 0;
+#pragma unroll
+                for (int dx = LD; dx >= 0; --dx)
+#pragma unroll
+                for (int dy = LD - dx; dy >= 0; --dy) {
+                  const int dz = LD - dx - dy;
+                  g[ps][cl * ND + d] = fma(X[ocx[cl] + dx] * Y[ocy[cl] + dy], Z[ocz[cl] + dz], g[ps][cl * ND + d]);
+                  ++d;
+                }
+              }
+            } else {
             int cd = 0;
 #pragma unroll
             for (int cx = LC; cx >= 0; --cx)
@@ -273,6 +301,7 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
               const int cz = LC - cx - cy, dz = LD - dx - dy;
               g[ps][cd] = fma(X[cx * (LD + 1) + dx] * Y[cy * (LD + 1) + dy], Z[cz * (LD + 1) + dz], g[ps][cd]);
               ++cd;
+            }
             }
           }
         }
@@ -342,19 +371,19 @@ __global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
   }
 }
 
-template <int LA, int LB, int LC, int LD, int TW>
+template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
 cudaError_t launch_coop_jk(const Work& w, int nblocks_dense, cudaStream_t s) {
-  using Tr = CoopTraits<LA, LB, LC, LD, TW>;
+  using Tr = CoopTraits<LA, LB, LC, LD, TW, NCH>;
   const int total = w.list ? (w.nlist + Tr::GROUPS - 1) / Tr::GROUPS : nblocks_dense;
   const int grid = (total + w.nshard - 1) / w.nshard;
   if (grid <= 0) return cudaSuccess;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(coop_jk_kernel<LA, LB, LC, LD, TW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(coop_jk_kernel<LA, LB, LC, LD, TW, NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  coop_jk_kernel<LA, LB, LC, LD, TW><<<grid, dim3(Tr::T, Tr::GROUPS), Tr::SMEM, s>>>(w);
+  coop_jk_kernel<LA, LB, LC, LD, TW, NCH><<<dim3(grid, NCH), dim3(Tr::T, Tr::GROUPS), Tr::SMEM, s>>>(w);
   return cudaGetLastError();
 }
 

@@ -22,7 +22,7 @@ static_assert(COOP_NGROUPS == 8, "tuned.cu lists eight cooperative groups");
 // warps per quartet of a cooperative class, 0 if the class is not served
 static int coop_tw(int key) {
   switch (key) {
-#define X(a, b, c, d, tw) case a * 1000 + b * 100 + c * 10 + d: return tw;
+#define X(a, b, c, d, tw, nch) case a * 1000 + b * 100 + c * 10 + d: return tw;
     COOP_ALL(X)
 #undef X
     default: return 0;

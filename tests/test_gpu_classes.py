@@ -14,7 +14,8 @@ torch = pytest.importorskip("torch")
 from paper_2407_09700_b200 import workloads as W  # noqa: E402
 
 CLASSES_F = [c for c in W.canonical_classes(4) if max(c) <= 3]
-CLASSES_G = [(4, 0, 0, 0), (4, 1, 1, 0), (4, 0, 2, 0), (4, 2, 2, 1), (4, 3, 1, 0), (4, 4, 2, 0), (4, 1, 4, 1), (4, 4, 3, 2), (4, 3, 4, 3)]
+CLASSES_G = [(4, 0, 0, 0), (4, 1, 1, 0), (4, 0, 2, 0), (4, 2, 2, 1), (4, 3, 1, 0), (4, 4, 2, 0), (4, 1, 4, 1), (4, 4, 3, 2), (4, 3, 4, 3),
+             (4, 3, 3, 3), (4, 4, 4, 2), (4, 4, 4, 4)]   # the last four: ket components of shell c in chunks (coop_kernel.cuh, NCH > 1)
 
 
 @pytest.fixture(scope="module")
@@ -58,6 +59,8 @@ def test_tuned_kernels_are_selected(eri):
         kinds.setdefault((c["la"], c["lb"], c["lc"], c["ld"]), set()).add(c["kernel"])
     assert all(k.issubset({1, 2, 3}) for k in kinds.values()), kinds
     assert kinds[(3, 3, 3, 3)] == {2}
+    lp = eri.eri_list_plan_create(*W.cfg1_class((4, 4, 4, 4), 1, nquartets=4, pool=4)[::2])
+    assert {c["kernel"] for c in lp.class_stats()} == {2}   # no class is left on the generic kernel
     plan.set_kernel_mode(2)   # register and cooperative families only
     kinds = {}
     for c in plan.class_stats():
