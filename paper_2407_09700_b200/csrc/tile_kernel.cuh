@@ -122,19 +122,24 @@ template <int NV, bool HALVES, class F>
 __device__ __forceinline__ void warp_reduce_values(const double* __restrict__ v, double* __restrict__ stage, int lane, F emit) {
   if constexpr (NV <= 16) {
     // few values: all 32 lanes work.  ROWS value-rows x LPR lanes per row; a lane adds ROWS staged elements of its row
-    // (interleaved, within its ket half if HALVES), then the LPR (LPR/2) lanes of a row (half) finish with shuffles.
+    // (within its ket half if HALVES), then the LPR (LPR/2) lanes of a row (half) finish with shuffles.
     constexpr int ROWS = NV <= 1 ? 1 : NV <= 2 ? 2 : NV <= 4 ? 4 : NV <= 8 ? 8 : 16;
-    constexpr int LPR = 32 / ROWS, GRP = HALVES ? LPR / 2 : LPR;   // lanes that share one sum
+    constexpr int LPR = 32 / ROWS, GRP = HALVES ? LPR / 2 : LPR;   // lanes per row; lanes that share one sum
+    constexpr int RS = 32 + LPR;                                    // row stride: lane id == bank (mod 16) on both sides
+    // staged position of the value of source lane L: the elements of ket half h land on the columns that the lanes of
+    // half h read (column mod LPR in [h GRP, (h+1) GRP)), so that lane sl of a row simply reads columns sl + m LPR
+    const int q = lane & 15, hl = lane >> 4;
+    const int pos = HALVES ? (q / GRP) * LPR + hl * GRP + (q % GRP) : lane;
     __syncwarp();
 #pragma unroll
-    for (int i = 0; i < NV; ++i) stage[i * 33 + lane] = v[i];
+    for (int i = 0; i < NV; ++i) stage[i * RS + pos] = v[i];
     __syncwarp();
     const int row = lane / LPR, sl = lane - row * LPR;
     const int half = HALVES ? sl / GRP : 0, t = sl - half * GRP;
-    const double* src = stage + row * 33 + 16 * half + t;
+    const double* src = stage + row * RS + sl;
     double sum = 0.0;
 #pragma unroll
-    for (int m = 0; m < ROWS; ++m) sum += src[m * GRP];
+    for (int m = 0; m < ROWS; ++m) sum += src[m * LPR];
 #pragma unroll
     for (int o = GRP / 2; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
     if (t == 0 && row < NV && sum != 0.0) emit(row, half, sum);
