@@ -116,6 +116,8 @@ struct CoopTraits {
   static_assert(ncart(LC) % NCH == 0, "NCH must divide the number of Cartesian components of shell c");
   static constexpr int NAB = NA * NB, NCD = NC * ND;
   static constexpr int PASSES = (NAB + T - 1) / T;
+  // three blocks per SM (170 registers) pay off for the classes with 16-20 accumulators per lane (measured on cfg3), not elsewhere
+  static constexpr int MINB = (PASSES * NCD >= 16 && PASSES * NCD <= 20) ? 3 : 0;   // 0 = unspecified (the compiler default keeps occupancy higher than an explicit 1)
   static constexpr int N = nroots_of(LA + LB + LC + LD);
   // strides of the slab: SCD = one (i,j) row, G2 = one (axis, root) block; both padded to odd so that lanes that differ in
   // (i,j) (phase 2 loads) or in (axis, root) (phase 1 stores) fall into different shared-memory banks
@@ -128,7 +130,7 @@ struct CoopTraits {
 };
 
 template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
-__global__ void __launch_bounds__(32 * COOP_WARPS) coop_jk_kernel(Work w) {
+__global__ void __launch_bounds__(32 * COOP_WARPS, (CoopTraits<LA, LB, LC, LD, TW, NCH>::MINB)) coop_jk_kernel(Work w) {
   using Tr = CoopTraits<LA, LB, LC, LD, TW, NCH>;
   constexpr int T = Tr::T, GROUPS = Tr::GROUPS;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
