@@ -177,13 +177,17 @@ struct TileTraits {
   static constexpr int N = nroots_of(LA + LB + LC + LD);
   static constexpr int G2 = (LA + 1) * (LB + 1) * (LC + 1) * (LD + 1);
   static constexpr int NW = BI * TQ, NT = 32 * NW;          // BI = quartet warps per block
+  // blocks per SM asked of the compiler (0 = unspecified), by block size and register demand RW = accumulators + 2-D integrals of
+  // one root; fitted to per-class timings on cfg3: more resident warps pay off until the tighter register cap makes the kernel spill
+  static constexpr int RW = NE + 3 * G2;
+  static constexpr int MINB = (NT == 128 && RW <= 63) ? 3 : (NT == 256 && TQ == 1 && RW >= 30) ? 2 : 0;
   static constexpr int NKEEP = NCD + NAT * ND;              // per-thread sums kept over the rows: J_cd, K_ad
   static constexpr int STAGE = 32 * 33;                     // doubles per warp
   static constexpr size_t SMEM = sizeof(double) * (NW * STAGE + NKEEP * NT);
 };
 
 template <int LA, int LB, int LC, int LD, int TQ, int BI>
-__global__ void __launch_bounds__(32 * BI * TQ) tile_jk_kernel(Work w) {
+__global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, BI>::MINB)) tile_jk_kernel(Work w) {
   using Tr = TileTraits<LA, LB, LC, LD, TQ, BI>;
   constexpr int NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAT = Tr::NAT, NABT = Tr::NABT, NCD = Tr::NCD, NE = Tr::NE;
   constexpr int N = Tr::N, G2 = Tr::G2, NT = Tr::NT, NKEEP = Tr::NKEEP;
