@@ -33,7 +33,7 @@ struct CoopGradTraits {
 };
 
 template <int LA, int LB, int LC, int LD, int WARPS>
-__global__ void __launch_bounds__(32 * WARPS) coop_grad_kernel(Work w) {
+__global__ void __launch_bounds__(32 * WARPS, ((WARPS == 4 && LD == 0 && LC >= 1 && LC <= 2 && ncart(LA) * ncart(LB) >= 18) ? 3 : 0)) coop_grad_kernel(Work w) {   // three blocks per SM where measured faster (cfg4)
   using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS>;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
   constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2;
