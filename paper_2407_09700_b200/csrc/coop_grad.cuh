@@ -18,7 +18,11 @@ namespace eri {
 
 constexpr int CGRAD_CH = 16;      // bra pairs per task
 
-template <int LA, int LB, int LC, int LD, int WARPS>   // WARPS = ket pairs per block (gen_class_lists.py sizes it for 200 KB of shared memory)
+// WARPS = ket pairs per block (gen_class_lists.py sizes it for 200 KB of shared memory).  EM = element mode of phase 2: the
+// Cartesian elements (a,b,c,d) are dealt over the 32 lanes one by one (run-time component indices, density blocks staged in
+// shared memory) instead of one bra component pair per lane -- for the classes whose nc(la) nc(lb) fills the lanes badly
+// ((dp|, (dd|, (fs| ...: 18, 36, 10 pairs).  There is no per-element accumulator, so any distribution of the elements works.
+template <int LA, int LB, int LC, int LD, int WARPS, int EM>
 struct CoopGradTraits {
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
   static constexpr int NAB = NA * NB, NCD = NC * ND;
@@ -26,15 +30,17 @@ struct CoopGradTraits {
   static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
   static constexpr int SCD = ((LC + 2) * (LD + 1)) | 1, G2 = ((LA + 2) * (LB + 2) * SCD) | 1;   // raised on A, B, C; odd strides: no bank conflicts
   static constexpr int SLAB2D = 3 * N * G2;
-  static constexpr int SLAB = (SLAB2D > 32 * 33 ? SLAB2D : 32 * 33) + NCD;          // + staged D_cd
+  static constexpr int BASE = SLAB2D > 32 * 33 ? SLAB2D : 32 * 33;
+  static constexpr int NDQ = EM ? NAB + NA * NC + NA * ND + NB * NC + NB * ND : 0;   // D_ab, D_ac, D_ad, D_bc, D_bd of the quartet (element mode)
+  static constexpr int SLAB = BASE + NDQ + NCD;                                      // + staged D_cd
   static constexpr size_t SMEM = sizeof(double) * SLAB * WARPS;
   static_assert(SMEM <= 227 * 1024, "slab does not fit");
   static_assert(3 * N <= 32, "one lane per (root, axis)");
 };
 
-template <int LA, int LB, int LC, int LD, int WARPS>
-__global__ void __launch_bounds__(32 * WARPS, ((WARPS == 4 && LD == 0 && LC >= 1 && LC <= 2 && ncart(LA) * ncart(LB) >= 18) ? 3 : 0)) coop_grad_kernel(Work w) {   // three blocks per SM where measured faster (cfg4)
-  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS>;
+template <int LA, int LB, int LC, int LD, int WARPS, int EM>
+__global__ void __launch_bounds__(32 * WARPS, ((EM == 0 && WARPS == 4 && LD == 0 && LC >= 1 && LC <= 2 && ncart(LA) * ncart(LB) >= 18) ? 3 : 0)) coop_grad_kernel(Work w) {   // three blocks per SM where measured faster (cfg4)
+  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS, EM>;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;
   constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2;
   constexpr int SL = 1, SK = LD + 1, SJ = SCD, SI = (LB + 2) * SCD;   // strides of (i, j, k, l) in the slab
@@ -42,6 +48,7 @@ __global__ void __launch_bounds__(32 * WARPS, ((WARPS == 4 && LD == 0 && LC >= 1
   const int lane = threadIdx.x, wy = threadIdx.y;
   double* S = smem + (size_t)wy * Tr::SLAB;
   double* sDcd = S + (Tr::SLAB - NCD);
+  double* sDab = S + Tr::BASE; double* sDac = sDab + NAB; double* sDad = sDac + NA * NC; double* sDbc = sDad + NA * ND; double* sDbd = sDbc + NB * NC;   // element mode
 
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
@@ -74,6 +81,15 @@ __global__ void __launch_bounds__(32 * WARPS, ((WARPS == 4 && LD == 0 && LC >= 1
 #pragma unroll
     for (int x = 0; x < 3; ++x) { A[x] = bp.geom[x * bp.stride + i]; AB[x] = bp.geom[(3 + x) * bp.stride + i]; }
     const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
+    if constexpr (EM != 0) {
+      __syncwarp();
+      for (int e = lane; e < NAB; e += 32) sDab[e] = D[(long)(a0 + e / NB) * n + b0 + e % NB];
+      for (int e = lane; e < NA * NC; e += 32) sDac[e] = D[(long)(a0 + e / NC) * n + c0 + e % NC];
+      for (int e = lane; e < NA * ND; e += 32) sDad[e] = D[(long)(a0 + e / ND) * n + d0 + e % ND];
+      for (int e = lane; e < NB * NC; e += 32) sDbc[e] = D[(long)(b0 + e / NC) * n + c0 + e % NC];
+      for (int e = lane; e < NB * ND; e += 32) sDbd[e] = D[(long)(b0 + e / ND) * n + d0 + e % ND];
+      __syncwarp();
+    }
 
     double acc[18];   // [J: A xyz, B xyz, C xyz | K: same]
 #pragma unroll
@@ -133,6 +149,41 @@ __global__ void __launch_bounds__(32 * WARPS, ((WARPS == 4 && LD == 0 && LC >= 1
         }
         __syncwarp();
         // ---- phase 2 ----
+        if constexpr (EM != 0) {
+#pragma unroll 1
+          for (int e = lane; e < NAB * NCD; e += 32) {
+            const int id = e % ND, t1 = e / ND, ic = t1 % NC, t2 = t1 / NC, ib = t2 % NB, ia = t2 / NB;
+            int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
+            cart_powers(LA, ia, ax, ay, az); cart_powers(LB, ib, bx, by, bz); cart_powers(LC, ic, cx, cy, cz); cart_powers(LD, id, dx, dy, dz);
+            const double pj = sDab[ia * NB + ib] * sDcd[ic * ND + id];
+            const double pk = fma(sDac[ia * NC + ic], sDbd[ib * ND + id], sDad[ia * ND + id] * sDbc[ib * NC + ic]);
+            const int ox = ax * SI + bx * SJ + cx * SK + dx, oy = ay * SI + by * SJ + cy * SK + dy + N * G2, oz = az * SI + bz * SJ + cz * SK + dz + 2 * N * G2;
+            // lowered terms vanish with their integer factor; the slab has no index -1, so the offset is 0 there
+            const int lax = ax > 0 ? -SI : 0, lay = ay > 0 ? -SI : 0, laz = az > 0 ? -SI : 0;
+            const int lbx = bx > 0 ? -SJ : 0, lby = by > 0 ? -SJ : 0, lbz = bz > 0 ? -SJ : 0;
+            const int lcx = cx > 0 ? -SK : 0, lcy = cy > 0 ? -SK : 0, lcz = cz > 0 ? -SK : 0;
+            const double fax = ax, fay = ay, faz = az, fbx = bx, fby = by, fbz = bz, fcx = cx, fcy = cy, fcz = cz;
+#pragma unroll 1
+            for (int rt = 0; rt < N; ++rt) {
+              const double* X = S + ox + rt * G2;
+              const double* Y = S + oy + rt * G2;
+              const double* Z = S + oz + rt * G2;
+              const double vx = X[0], vy = Y[0], vz = Z[0];
+              const double oyz = vy * vz, oxz = vx * vz, oxy = vx * vy;
+              const double dAx = fma(ea2, X[SI], -fax * X[lax]), dAy = fma(ea2, Y[SI], -fay * Y[lay]), dAz = fma(ea2, Z[SI], -faz * Z[laz]);
+              const double dBx = fma(eb2, X[SJ], -fbx * X[lbx]), dBy = fma(eb2, Y[SJ], -fby * Y[lby]), dBz = fma(eb2, Z[SJ], -fbz * Z[lbz]);
+              const double dCx = fma(ec2, X[SK], -fcx * X[lcx]), dCy = fma(ec2, Y[SK], -fcy * Y[lcy]), dCz = fma(ec2, Z[SK], -fcz * Z[lcz]);
+              const double jx = pj * oyz, jy = pj * oxz, jz = pj * oxy;
+              const double kx = pk * oyz, ky = pk * oxz, kz = pk * oxy;
+              acc[0] = fma(dAx, jx, acc[0]); acc[1] = fma(dAy, jy, acc[1]); acc[2] = fma(dAz, jz, acc[2]);
+              acc[3] = fma(dBx, jx, acc[3]); acc[4] = fma(dBy, jy, acc[4]); acc[5] = fma(dBz, jz, acc[5]);
+              acc[6] = fma(dCx, jx, acc[6]); acc[7] = fma(dCy, jy, acc[7]); acc[8] = fma(dCz, jz, acc[8]);
+              acc[9] = fma(dAx, kx, acc[9]); acc[10] = fma(dAy, ky, acc[10]); acc[11] = fma(dAz, kz, acc[11]);
+              acc[12] = fma(dBx, kx, acc[12]); acc[13] = fma(dBy, ky, acc[13]); acc[14] = fma(dBz, kz, acc[14]);
+              acc[15] = fma(dCx, kx, acc[15]); acc[16] = fma(dCy, ky, acc[16]); acc[17] = fma(dCz, kz, acc[17]);
+            }
+          }
+        } else
 #pragma unroll
         for (int ps = 0; ps < PASSES; ++ps) {
           int ab = lane + 32 * ps;
@@ -224,18 +275,18 @@ __global__ void __launch_bounds__(32 * WARPS, ((WARPS == 4 && LD == 0 && LC >= 1
   }
 }
 
-template <int LA, int LB, int LC, int LD, int WARPS>
+template <int LA, int LB, int LC, int LD, int WARPS, int EM>
 cudaError_t launch_coop_grad(const Work& w, int nblocks_dense, cudaStream_t s) {
-  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS>;
+  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS, EM>;
   const int grid = (nblocks_dense + w.nshard - 1) / w.nshard;
   if (grid <= 0) return cudaSuccess;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(coop_grad_kernel<LA, LB, LC, LD, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(coop_grad_kernel<LA, LB, LC, LD, WARPS, EM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  coop_grad_kernel<LA, LB, LC, LD, WARPS><<<grid, dim3(32, WARPS), Tr::SMEM, s>>>(w);
+  coop_grad_kernel<LA, LB, LC, LD, WARPS, EM><<<grid, dim3(32, WARPS), Tr::SMEM, s>>>(w);
   return cudaGetLastError();
 }
 
