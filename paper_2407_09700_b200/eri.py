@@ -110,7 +110,10 @@ class Plan:
         self._h, self.basis, self.is_list = handle, basis, is_list
 
     def __del__(self):
-        self.destroy()
+        try:
+            self.destroy()
+        except Exception:   # interpreter shutdown: the module globals may already be gone; the process is ending anyway
+            pass
 
     def destroy(self):
         if getattr(self, "_h", None):
