@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(32 * WARPS, ((EM == 0 && WARPS == 4 && LD == 0
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
   if (blk >= w.row_off[w.nrows]) return;
-  const int r = find_row(w.row_off, w.nrows, blk);
+  const int r = find_row_warp(w.row_off, w.nrows, blk, threadIdx.x);
   const int j = (blk - w.row_off[r]) * WARPS + wy;
   const int i_begin = r * CGRAD_CH, i_end = min(i_begin + CGRAD_CH, bp.npair);
   if (j >= kp.npair) return;

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(32 * COOP_WARPS, (CoopTraits<LA, LB, LC, LD, T
     i_begin = w.list[t].x; i_end = i_begin + 1; j = w.list[t].y;
   } else {
     if (blk >= w.row_off[w.nrows]) return;
-    const int r = find_row(w.row_off, w.nrows, blk);
+    const int r = find_row_warp(w.row_off, w.nrows, blk, threadIdx.x & 31);
     j = (blk - w.row_off[r]) * GROUPS + wy;
     i_begin = r * COOP_CH; i_end = min(i_begin + COOP_CH, bp.npair);
     if (j >= kp.npair) return;

@@ -128,4 +128,19 @@ __device__ __forceinline__ int find_row(const int* __restrict__ row_off, int nro
   return lo;
 }
 
+// the same with the 32 lanes of a warp probing 32 pivots per round (3 rounds of dependent loads instead of 13 for 8192 rows);
+// every lane returns the row.  Must be called by all lanes of the warp.
+__device__ __forceinline__ int find_row_warp(const int* __restrict__ row_off, int nrows, int b, int lane) {
+  int lo = 0, hi = nrows;   // invariant: row_off[lo] <= b < row_off[hi]
+  while (hi - lo > 1) {
+    const int stride = (hi - lo + 31) >> 5;
+    const int idx = lo + lane * stride;
+    const bool le = idx < hi && row_off[idx] <= b;
+    const int t = __popc(__ballot_sync(0xffffffffu, le));   // lanes 0 .. t-1 are true (row_off is non-decreasing), t >= 1
+    lo += (t - 1) * stride;
+    hi = min(hi, lo + stride);
+  }
+  return lo;
+}
+
 }  // namespace eri

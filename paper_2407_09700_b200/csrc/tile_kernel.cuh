@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
   if (blk >= w.row_off[w.nrows]) return;
-  const int r = find_row(w.row_off, w.nrows, blk);
+  const int r = find_row_warp(w.row_off, w.nrows, blk, threadIdx.x);
   const int x = threadIdx.x, wy = threadIdx.y, gq = wy / TQ, t = wy - gq * TQ, tid = wy * 32 + x;
   const int i_first = w.row_slot[r], j_first = (blk - w.row_off[r]) * 32;
   double* stage = smem + wy * Tr::STAGE;
