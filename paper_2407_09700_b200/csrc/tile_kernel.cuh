@@ -169,6 +169,14 @@ __device__ __forceinline__ void warp_reduce_values(const double* __restrict__ v,
   }
 }
 
+// doubles of warp-private staging that warp_reduce_values<NV> touches
+__host__ __device__ constexpr int reduce_stage_size(int nv) {
+  if (nv > 16) return 32 * 33;
+  const int rows = nv <= 1 ? 1 : nv <= 2 ? 2 : nv <= 4 ? 4 : nv <= 8 ? 8 : 16;
+  return rows * (32 + 32 / rows);
+}
+__host__ __device__ constexpr int max3(int a, int b, int c) { return a > b ? (a > c ? a : c) : (b > c ? b : c); }
+
 template <int LA, int LB, int LC, int LD, int TQ, int BI>
 struct TileTraits {
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
@@ -180,9 +188,9 @@ struct TileTraits {
   // blocks per SM asked of the compiler (0 = unspecified), by block size and register demand RW = accumulators + 2-D integrals of
   // one root; fitted to per-class timings on cfg3: more resident warps pay off until the tighter register cap makes the kernel spill
   static constexpr int RW = NE + 3 * G2;
-  static constexpr int MINB = (NT == 128 && RW <= 63) ? 3 : (NT == 256 && TQ == 1 && RW >= 30) ? 2 : 0;
+  static constexpr int MINB = (NT == 128 && RW <= 63) ? 3 : (NT == 256 && TQ == 1 && RW >= 30) ? 2 : (NT == 256 && RW <= 15) ? 4 : 0;
   static constexpr int NKEEP = NCD + NAT * ND;              // per-thread sums kept over the rows: J_cd, K_ad
-  static constexpr int STAGE = 32 * 33;                     // doubles per warp
+  static constexpr int STAGE = max3(reduce_stage_size(NABT), reduce_stage_size(NAT * NC), reduce_stage_size(NB * NC));   // doubles per warp
   static constexpr size_t SMEM = sizeof(double) * (NW * STAGE + NKEEP * NT);
 };
 
