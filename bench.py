@@ -253,13 +253,13 @@ def main():
     kern_ms = sum(c[key] for c in classes)
     top = max(classes, key=lambda c: c[key]) if classes else None
     achieved = flops / world / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0
-    # DRAM traffic of the dominant launch from its `ncu --set full` capture (profiles/r01c_cfg3.md): only known for the launch
+    # DRAM traffic of the dominant launch from its `ncu --set full` capture (profiles/r01d_cfg3.md): only known for the launch
     # that was captured, the (dp|dp) K = 1 unit of cfg3 (dram__bytes_read.sum + dram__bytes_write.sum = 48.0 + 137.0 MB)
     traffic = None
     if top is not None and kind == "jk" and args.workload == "cfg3" and [top["la"], top["lb"], top["lc"], top["ld"], top["ka"], top["kb"], top["kc"], top["kd"]] == [2, 1, 2, 1, 1, 1, 1, 1]:
         traffic = 185.0e6
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak if fp64_peak else None,
-                "traffic": traffic, "traffic_note": "bytes per launch of top_class (ncu --set full, profiles/r01c_cfg3.md); null when that launch was not captured", "peak_source": "FP64 DFMA rate measured in this run (eri_measure_fp64_peak); nominal "
+                "traffic": traffic, "traffic_note": "bytes per launch of top_class (ncu --set full, profiles/r01d_cfg3.md); null when that launch was not captured", "peak_source": "FP64 DFMA rate measured in this run (eri_measure_fp64_peak); nominal "
                 f"{NOMINAL_FP64_TFLOPS:.1f} = 148 SMs x 64 lanes x 2 x 1.965 GHz", "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
                 "kernel": "all class kernels of one step (canonical FLOPs of the kept quartets / summed device time of the class launches, measured in one extra serialised step with an event between launches)",
                 "class_kernels_share_of_step": kern_ms / ms if ms else None,
