@@ -92,6 +92,10 @@ def test_cfg3_kernel_selections_and_schedules_agree(eri, cfg3_jk):
     assert 3 in kinds and 2 in kinds and 0 not in kinds          # no class of cfg3 is left on the generic kernel
     st = plan.stats()
     assert st["quartets_kept"] == sum(c["quartets"] for c in plan.class_stats())
+    # lane slots swept by a launch cover its quartets; the shell-grouped tiles of the tile family are well filled
+    assert all(c["slots"] >= c["quartets"] for c in plan.class_stats())
+    tile = [c for c in plan.class_stats() if c["kernel"] == 3]
+    assert sum(c["quartets"] for c in tile) >= 0.75 * sum(c["slots"] for c in tile)
     plan.set_timing(True)                                         # serialised schedule
     J1, K1 = plan.build_jk(dev(D))
     plan.set_timing(False)
