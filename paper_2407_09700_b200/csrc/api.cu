@@ -300,6 +300,7 @@ int schwarz_of_class(PairClass& pc, cudaStream_t s) {
 // tile family only where at least TILE_MIN_FILL of the swept lanes has work and the bra chunks hold enough rows to amortise
 // the block-end reduction (measured on cfg3)
 constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3, TILE_MIN_FILL_COOP = 0.25, TILE_MIN_FILL_GRAD = 0.1;
+constexpr long long COOP_GRAD_MIN_TASKS = 4096;   // about two waves of 12 warps on 148 SMs
 constexpr double HRR_LOSS_MAX_GRAD = 1.0e5;   // gradient tolerance is 1e-8 Ha/Bohr absolute
 constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
 
@@ -449,6 +450,9 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
   // cooperative gradient kernel for what the tile gradient kernel does not serve (it chooses the build centre itself)
   if (pl.kernel_mode != 1 && pl.want_grad && canonical && !pl.is_list && u.kernel_grad == 0 && coop_grad_info(P.la, P.lb, R.la, R.lb, &ti)) {
     u.kernel_grad = 2; u.gBI = ti.BI; u.gBJ = ti.BJ;
+    // a warp walks its task's bra pairs one after the other: units of few, heavy quartets (the contracted core shells,
+    // K^4 = 4096 primitive quartets each) get shorter runs so that they still spread over the SMs
+    while (u.gBI > 1 && u.quartets / u.gBI < COOP_GRAD_MIN_TASKS) u.gBI /= 2;
   }
   if (!pl.is_list) {
     std::vector<int> ro;
@@ -472,6 +476,7 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
   w.row_off = grad ? u.g_row_off.p : u.row_off.p;
   w.nrows = grad ? u.g_nrows : u.nrows;
   w.thr = pl.thr;
+  w.grad_ch = u.gBI;
   if (grad ? u.kernel_grad == 3 : u.kernel == 3) {
     w.bra = pl.pcs[u.P]->grouped->view(); w.ket = pl.pcs[u.R]->grouped->view();
     w.row_off = u.t_row_off.p; w.row_slot = u.t_row_slot.p; w.nrows = u.t_nrows;

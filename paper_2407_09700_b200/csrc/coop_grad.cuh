@@ -16,7 +16,7 @@
 
 namespace eri {
 
-constexpr int CGRAD_CH = 16;      // bra pairs per task
+constexpr int CGRAD_CH = 16;      // bra pairs per task (the host shortens the run, Work::grad_ch, for units of few heavy quartets)
 
 // WARPS = ket pairs per block (gen_class_lists.py sizes it for 200 KB of shared memory).  EM = element mode of phase 2: the
 // Cartesian elements (a,b,c,d) are dealt over the 32 lanes one by one (run-time component indices, density blocks staged in
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(32 * WARPS, ((EM == 0 && WARPS == 4 && LD == 0
   if (blk >= w.row_off[w.nrows]) return;
   const int r = find_row_warp(w.row_off, w.nrows, blk, threadIdx.x);
   const int j = (blk - w.row_off[r]) * WARPS + wy;
-  const int i_begin = r * CGRAD_CH, i_end = min(i_begin + CGRAD_CH, bp.npair);
+  const int i_begin = r * w.grad_ch, i_end = min(i_begin + w.grad_ch, bp.npair);
   if (j >= kp.npair) return;
   const int n = w.nao;
   const double* __restrict__ D = w.D;

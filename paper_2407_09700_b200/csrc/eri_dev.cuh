@@ -114,6 +114,7 @@ struct Work {
   // chunks; a quartet is evaluated iff q_i * q_j >= thr (and j <= i when bra set == ket set) -- the same set as dense mode.
   const int* row_slot;
   double thr;
+  int grad_ch;       // cooperative gradient kernel: bra pairs per task (Unit::gBI)
 };
 
 __device__ __forceinline__ void atomic_add(double* p, double v) { atomicAdd(p, v); }
