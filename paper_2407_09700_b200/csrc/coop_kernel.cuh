@@ -13,7 +13,7 @@
 //            that share a resp. b through the (now dead) slab, and leave as one FP64 atomic per block element;
 //            J_cd is summed in registers over the bra pairs of the warp's task and reduced across lanes once per task.
 // A task is one ket pair and a run of CH consecutive bra pairs of the Schwarz-sorted tile row.
-// Large classes give a quartet to TW = 2 or 4 warps (a "group", synchronised with a named barrier) so that the
+// Large classes give a quartet to TW = 2, 4 or 8 warps (a "group", synchronised with a named barrier) so that the
 // accumulators per lane, ceil(nab / 32 TW) * ncd, stay in registers.
 #pragma once
 #include "eri_dev.cuh"
@@ -111,7 +111,8 @@ __device__ __forceinline__ void group_sync(int tw, int id) {
 // the 2-D integrals are then rebuilt once per chunk (cheap next to the products of such classes).
 template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
 struct CoopTraits {
-  static constexpr int T = 32 * TW, GROUPS = COOP_WARPS / TW;
+  static constexpr int WARPS = TW > COOP_WARPS ? TW : COOP_WARPS;   // TW = 8: the block is one group of eight warps (slab-bound classes)
+  static constexpr int T = 32 * TW, GROUPS = WARPS / TW;
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC) / NCH, ND = ncart(LD);   // NC: components of c per chunk
   static_assert(ncart(LC) % NCH == 0, "NCH must divide the number of Cartesian components of shell c");
   static constexpr int NAB = NA * NB, NCD = NC * ND;
@@ -130,7 +131,7 @@ struct CoopTraits {
 };
 
 template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
-__global__ void __launch_bounds__(32 * COOP_WARPS, (CoopTraits<LA, LB, LC, LD, TW, NCH>::MINB)) coop_jk_kernel(Work w) {
+__global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WARPS), (CoopTraits<LA, LB, LC, LD, TW, NCH>::MINB)) coop_jk_kernel(Work w) {
   using Tr = CoopTraits<LA, LB, LC, LD, TW, NCH>;
   constexpr int T = Tr::T, GROUPS = Tr::GROUPS;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD, PASSES = Tr::PASSES;

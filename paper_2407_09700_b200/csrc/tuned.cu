@@ -42,7 +42,7 @@ static bool is_reg_class(int key) {
 bool tuned_jk_info(int la, int lb, int lc, int ld, int, int, TunedInfo* info) {
   const int key = la * 1000 + lb * 100 + lc * 10 + ld;
   if (is_reg_class(key)) { info->kind = 1; info->BI = 4; info->BJ = 32; return true; }
-  if (const int tw = coop_tw(key)) { info->kind = 2; info->BI = 16; info->BJ = 4 / tw; return true; }   // COOP_CH bra pairs x (COOP_WARPS / TW) ket pairs
+  if (const int tw = coop_tw(key)) { info->kind = 2; info->BI = 16; info->BJ = tw > 4 ? 1 : 4 / tw; return true; }   // COOP_CH bra pairs x (max(COOP_WARPS, TW) / TW) ket pairs
   return false;
 }
 
