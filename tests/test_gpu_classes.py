@@ -15,7 +15,7 @@ from paper_2407_09700_b200 import workloads as W  # noqa: E402
 
 CLASSES_F = [c for c in W.canonical_classes(4) if max(c) <= 3]
 CLASSES_G = [(4, 0, 0, 0), (4, 1, 1, 0), (4, 0, 2, 0), (4, 2, 2, 1), (4, 3, 1, 0), (4, 4, 2, 0), (4, 1, 4, 1), (4, 4, 3, 2), (4, 3, 4, 3),
-             (4, 3, 3, 3), (4, 4, 4, 2), (4, 4, 4, 4)]   # the last four: ket components of shell c in chunks (coop_kernel.cuh, NCH > 1)
+             (4, 3, 3, 3), (4, 4, 4, 2), (4, 4, 4, 4), (4, 4, 3, 3), (4, 4, 4, 3)]   # the last six: ket components of shell c in chunks (coop_kernel.cuh, NCH > 1)
 
 
 @pytest.fixture(scope="module")
