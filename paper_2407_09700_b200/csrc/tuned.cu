@@ -119,6 +119,9 @@ cudaError_t launch_coop_grad_class(const Work& w, int nblocks, cudaStream_t s) {
 bool tuned_grad_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info) {
   // (dp|ps) spills (profiles/r01d_cfg4.md: 45 GB of local-memory traffic); over long primitive loops the cooperative kernel is faster
   if (la == 2 && lb == 1 && lc == 1 && ld == 0 && npp_bra * npp_ket >= 8) return false;
+  // few quartets with 24 primitive ket pairs (K = 3 x 8) fill the tile's 32 ket slots badly; measured on cfg4: faster on the cooperative kernel
+  // for the (x|ps) classes, slower for (x|ss) and for the contracted (ds|pp), (pp|pp) units (profiles/r01f_cfg4.md)
+  if (lc >= 1 && npp_ket >= 24) return false;
   switch (la * 1000 + lb * 100 + lc * 10 + ld) {
 #define X(a, b, c, d, bi, mode) case a * 1000 + b * 100 + c * 10 + d: info->kind = 3; info->TQ = 1; info->BI = bi; info->BJ = 32; return true;
     TGRAD_ALL(X)
