@@ -300,7 +300,7 @@ int schwarz_of_class(PairClass& pc, cudaStream_t s) {
 // tile family only where at least TILE_MIN_FILL of the swept lanes has work and the bra chunks hold enough rows to amortise
 // the block-end reduction (measured on cfg3)
 constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3, TILE_MIN_FILL_COOP = 0.25, TILE_MIN_FILL_GRAD = 0.1;
-constexpr long long COOP_GRAD_MIN_TASKS = 4096;   // about two waves of 12 warps on 148 SMs
+constexpr long long COOP_GRAD_MIN_TASKS = 32768;   // some twenty waves of 12 warps on 148 SMs: the tail of a unit is a wave of heavy tasks
 constexpr double HRR_LOSS_MAX_GRAD = 1.0e5;   // gradient tolerance is 1e-8 Ha/Bohr absolute
 constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
 
