@@ -90,6 +90,14 @@ def eri_block(basis, i, j, k, l, deriv: bool = False) -> np.ndarray:
     return out
 
 
+def overlap_block(basis, i, j) -> np.ndarray:
+    """<i|j> of two contracted spherical shells from the E_0 Hermite coefficients (a pin helper, see md_oracle.cpp)."""
+    out = np.zeros((2 * int(basis.shells["l"][i]) + 1, 2 * int(basis.shells["l"][j]) + 1))
+    args, keep = _basis_args(basis)
+    lib().oracle_overlap_block(*args, int(i), int(j), _d(out))
+    return out
+
+
 def schwarz(basis) -> np.ndarray:
     Q = np.zeros((basis.nshell, basis.nshell))
     args, keep = _basis_args(basis)

@@ -20,7 +20,9 @@
 // and mpmath quadrature, Gauss-Hermite x Gauss-Legendre brute-force quadrature of primitive ERIs up to
 // g functions, centre-derivative ladder, 8-fold symmetry, translational invariance, J/K symmetry and
 // linearity, R9 symmetry-list digestion == plain quadruple loop, gradient per-axis sums = 0 and central
-// finite differences of E_J, E_K.  Absolute J/K/gradient values on the synthetic clusters have no
+// finite differences of E_J, E_K; the contraction loop and the four-index Cartesian -> spherical transform for l >= 1
+// against contracted blocks assembled from brute-force quadrature components (test_contracted_spherical_block_vs_quadrature);
+// orthonormality of contracted spherical shells through the E_0 overlap (test_contracted_spherical_shells_are_orthonormal).  Absolute J/K/gradient values on the synthetic clusters have no
 // external reference ("parity unpinned" beyond this chain).
 
 #include <algorithm>
@@ -387,6 +389,30 @@ void oracle_eri_block(const int32_t* shells, int nsh, const double* prims, int n
   BasisView bv = view(shells, nsh, prims, npr, xyz, natm);
   PairData bra, ket; make_pair(bv, i, j, deriv ? 1 : 0, bra); make_pair(bv, k, l, 0, ket);
   Scratch s; shell_quartet(bra, ket, deriv != 0, out, s);
+}
+
+// Overlap block <i|j> of two contracted spherical shells from the E_0 Hermite coefficients (SURVEY 8(c) table "c2s matrices"):
+// S = sum_prims c_a c_b E_0^x E_0^y E_0^z (pi/p)^{3/2}, then the same index transform as shell_quartet on indices 0 and 1.
+// A pin helper: shells normalised by reading R2 must give the unit matrix for i == j.  out: [ns_i][ns_j].
+void oracle_overlap_block(const int32_t* shells, int nsh, const double* prims, int npr, const double* xyz, int natm,
+                          int i, int j, double* out) {
+  BasisView bv = view(shells, nsh, prims, npr, xyz, natm);
+  PairData pd; make_pair(bv, i, j, 0, pd);
+  const int la = pd.la, lb = pd.lb, na = ncart(la), nb = ncart(lb), nt = la + lb + 1;
+  std::vector<double> cart((size_t)na * nb, 0.0), half((size_t)nsph(la) * nb), full((size_t)nsph(la) * nsph(lb));
+  for (const PrimPair& pp : pd.pp)
+    for (int ia = 0; ia < na; ++ia)
+      for (int ib = 0; ib < nb; ++ib) {
+        int pa[3], pb[3]; cart_powers(la, ia, pa); cart_powers(lb, ib, pb);
+        double e0 = 1.0;
+        for (int x = 0; x < 3; ++x) e0 *= pp.E[x][((size_t)pa[x] * (lb + 1) + pb[x]) * nt];
+        cart[(size_t)ia * nb + ib] += pp.cc * e0 * std::pow(M_PI / pp.p, 1.5);
+      }
+  int dims[4] = {na, nb, 1, 1};
+  transform_index(cart.data(), half.data(), 1, dims, 0, g_c2s[la].data(), nsph(la));
+  dims[0] = nsph(la);
+  transform_index(half.data(), full.data(), 1, dims, 1, g_c2s[lb].data(), nsph(lb));
+  std::memcpy(out, full.data(), sizeof(double) * full.size());
 }
 
 // Schwarz factors Q_ij = max over spherical components |(ab|ab)|^(1/2) (Eq. 7).  Q: [nsh][nsh].

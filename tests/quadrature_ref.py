@@ -47,3 +47,38 @@ def prim_eri_quadrature(powers, exps, centres):
                                 A[x], B[x], C[x], D[x])
         total += wt * f * np.sqrt(rho) * (1.0 - t * t) ** -1.5
     return 2.0 / np.sqrt(np.pi) * total
+
+
+def cart_powers(l):
+    """Cartesian components of a shell in the order of reading R3: lx descending, then ly descending."""
+    return [(lx, ly, l - lx - ly) for lx in range(l, -1, -1) for ly in range(l - lx, -1, -1)]
+
+
+def prim_block_quadrature(ls, exps, centres):
+    """The whole Cartesian block [nc_a, nc_b, nc_c, nc_d] of one primitive quartet by the same quadrature: per node t
+    the three per-axis tables I[pa, pb, pc, pd] are formed once and every Cartesian component is a product of three
+    entries (the integrand factorises), so a block costs 3 * prod(l+1) axis integrals per node instead of 3 per component."""
+    la, lb, lc, ld = ls
+    a, b, c, d = exps
+    A, B, C, D = [np.asarray(x, dtype=float) for x in centres]
+    p, q = a + b, c + d
+    rho = p * q / (p + q)
+    pws = [cart_powers(l) for l in ls]
+    out = np.zeros([len(x) for x in pws])
+    ia = np.array([[pw[x] for pw in pws[0]] for x in range(3)])
+    ib = np.array([[pw[x] for pw in pws[1]] for x in range(3)])
+    ic = np.array([[pw[x] for pw in pws[2]] for x in range(3)])
+    id_ = np.array([[pw[x] for pw in pws[3]] for x in range(3)])
+    for t, wt in zip(_GL_X, _GL_W):
+        s2 = rho * t * t / (1.0 - t * t)
+        f = 1.0
+        for x in range(3):
+            tab = np.empty((la + 1, lb + 1, lc + 1, ld + 1))
+            for pa in range(la + 1):
+                for pb in range(lb + 1):
+                    for pc in range(lc + 1):
+                        for pd in range(ld + 1):
+                            tab[pa, pb, pc, pd] = _axis_integral(s2, pa, pb, pc, pd, a, b, c, d, A[x], B[x], C[x], D[x])
+            f = f * tab[ia[x][:, None, None, None], ib[x][None, :, None, None], ic[x][None, None, :, None], id_[x][None, None, None, :]]
+        out += wt * f * np.sqrt(rho) * (1.0 - t * t) ** -1.5
+    return 2.0 / np.sqrt(np.pi) * out

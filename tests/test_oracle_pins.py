@@ -17,7 +17,7 @@ import pytest
 from scipy.special import erf, gamma, gammainc
 
 from paper_2407_09700_b200 import workloads as W
-from quadrature_ref import prim_eri_quadrature
+from quadrature_ref import cart_powers, prim_block_quadrature, prim_eri_quadrature
 
 
 # ------------------------------------------------------------------------------------------------ Boys
@@ -179,6 +179,81 @@ def test_normalise_radial_integral():
         val, _ = quad(lambda r: r ** (2 * l + 2) * sum(ck * math.exp(-ek * r * r) for ck, ek in zip(c, e)) ** 2, 0, 30,
                       epsabs=1e-14, epsrel=1e-13, limit=400)
         assert val == pytest.approx(1.0, rel=1e-10)
+
+
+def _one_shell_basis(shells):
+    """shells: list of (l, exps, raw coefs, centre); every shell on its own atom"""
+    sh, pr, xyz, ao = [], [], [], 0
+    for ia, (l, e, c, ctr) in enumerate(shells):
+        sh.append((ia, l, len(e), len(pr), ao))
+        pr += [(float(ek), float(ck)) for ek, ck in zip(e, c)]
+        xyz.append(ctr)
+        ao += 2 * l + 1
+    return W.Basis(np.array(sh, dtype=W.SHELL_DTYPE), np.array(pr, dtype=W.PRIM_DTYPE), np.array(xyz, dtype=float), ao)
+
+
+def test_block_quadrature_matches_component_quadrature():
+    """the vectorised block quadrature of tests/quadrature_ref.py is the component quadrature that pins prim_eri"""
+    rng = np.random.default_rng(31)
+    ls = (2, 1, 1, 0)
+    ex = np.exp(rng.uniform(math.log(0.3), math.log(3.0), 4))
+    ctr = rng.uniform(-1.0, 1.0, (4, 3))
+    blk = prim_block_quadrature(ls, ex, ctr)
+    pws = [cart_powers(l) for l in ls]
+    for idx in [(0, 0, 0, 0), (3, 2, 1, 0), (5, 1, 2, 0), (2, 0, 0, 0)]:
+        pw = [pws[k][idx[k]] for k in range(4)]
+        assert blk[idx] == pytest.approx(prim_eri_quadrature(pw, ex, ctr), rel=1e-12)
+
+
+@pytest.mark.parametrize("ls,ks", [((1, 2, 3, 0), (2, 1, 1, 2)), ((2, 2, 1, 1), (1, 2, 2, 1)), ((4, 0, 1, 0), (2, 1, 2, 1)),
+                                   ((0, 3, 2, 1), (2, 2, 1, 1))])
+def test_contracted_spherical_block_vs_quadrature(orc, ls, ks):
+    """The oracle's contraction (Eq. 5) and its four-index Cartesian -> spherical transform (reading R3) for
+    l >= 1: expected block = einsum of brute-force quadrature primitive blocks with the RAW coefficients and the c2s
+    matrices, every Cartesian component from tests/quadrature_ref.py (no MD recurrence).  A transposed or mis-ordered
+    index in transform_index, a wrong component order or a dropped coefficient fails here; the shells have different l,
+    so no index permutation maps the block onto itself."""
+    from oracle import sph
+    rng = np.random.default_rng(700 + 37 * ls[0] + 11 * ls[1] + 5 * ls[2] + ls[3])
+    shells = []
+    for l, k in zip(ls, ks):
+        e = np.exp(rng.uniform(math.log(0.3), math.log(3.0), k))
+        shells.append((l, e, W.normalise(l, e, rng.uniform(0.3, 1.0, k) * rng.choice([-1.0, 1.0], k)), rng.uniform(-1.0, 1.0, 3)))
+    b = _one_shell_basis(shells)
+    cart = np.zeros([(l + 1) * (l + 2) // 2 for l in ls])
+    for ia, (ea, ca) in enumerate(zip(shells[0][1], shells[0][2])):
+        for ib, (eb, cb) in enumerate(zip(shells[1][1], shells[1][2])):
+            for ic, (ec, cc) in enumerate(zip(shells[2][1], shells[2][2])):
+                for id_, (ed, cd) in enumerate(zip(shells[3][1], shells[3][2])):
+                    cart += ca * cb * cc * cd * prim_block_quadrature(ls, [ea, eb, ec, ed], [s[3] for s in shells])
+    ref = np.einsum("abcd,ia,jb,kc,ld->ijkl", cart, sph.c2s(ls[0]), sph.c2s(ls[1]), sph.c2s(ls[2]), sph.c2s(ls[3]))
+    val = orc.eri_block(b, 0, 1, 2, 3)
+    assert val.shape == ref.shape
+    assert np.abs(val - ref).max() <= 1e-11 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("l", [0, 1, 2, 3, 4])
+def test_contracted_spherical_shells_are_orthonormal(orc, l):
+    """SURVEY 8(c) "c2s matrices" pin: a contracted shell normalised by reading R2 has unit self-overlap and its 2l+1
+    functions are orthonormal; the overlap comes from the oracle's E_0 Hermite coefficients, S = E0x E0y E0z (pi/p)^(3/2),
+    through the oracle's own index transform.  Two shells of different l on one centre are orthogonal; two displaced s
+    shells reproduce the closed-form Gaussian product overlap."""
+    rng = np.random.default_rng(900 + l)
+    e = np.exp(rng.uniform(-1.5, 2.5, 3))
+    c = W.normalise(l, e, rng.uniform(0.2, 1.0, 3))
+    l2 = (l + 2) % 5
+    e2 = np.exp(rng.uniform(-1.0, 1.0, 2))
+    c2 = W.normalise(l2, e2, rng.uniform(0.2, 1.0, 2))
+    ctr = rng.uniform(-1, 1, 3)
+    b = _one_shell_basis([(l, e, c, ctr), (l2, e2, c2, ctr)])
+    assert np.allclose(orc.overlap_block(b, 0, 0), np.eye(2 * l + 1), atol=1e-13)
+    assert np.allclose(orc.overlap_block(b, 1, 1), np.eye(2 * l2 + 1), atol=1e-13)
+    assert np.allclose(orc.overlap_block(b, 0, 1), 0.0, atol=1e-13)
+    if l == 0:
+        a1, a2, R = 0.8, 1.7, np.array([0.3, -0.4, 1.1])
+        bb = _one_shell_basis([(0, [a1], [1.0], np.zeros(3)), (0, [a2], [1.0], R)])
+        ref = (math.pi / (a1 + a2)) ** 1.5 * math.exp(-a1 * a2 / (a1 + a2) * R @ R) / (4 * math.pi)
+        assert orc.overlap_block(bb, 0, 1)[0, 0] == pytest.approx(ref, rel=1e-14)
 
 
 # ------------------------------------------------------------------------------------------------ ERI tensor invariants
