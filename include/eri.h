@@ -25,6 +25,12 @@
  * also blocks the host until its own device work is done.  The *_host entry points synchronise the stream before
  * returning.
  *
+ * Devices: the library binds to the CUDA device that is current at its first compute call (its Rys tables, the
+ * constant-memory transform table and the kernels' shared-memory attributes live there).  Calling any compute entry point
+ * while another device is current returns ERI_ERR_BAD_ARG; one process drives one GPU (multi-GPU: one process per GPU,
+ * eri_plan_set_shard).  eri_plan_set_kernel_mode re-uploads the plan's row tables and blocks the host until that is done
+ * (on a private stream: no device-wide synchronisation).
+ *
  * Errors: every int-returning function returns ERI_OK (0) or a negative code and never throws; the message of the
  * last failure in the calling thread is available through eri_last_error().  There is no CPU fallback: without a
  * CUDA device every compute entry point returns ERI_ERR_CUDA.
@@ -75,7 +81,7 @@ typedef struct {
   double canonical_flops;     /* per call                                                      */
   float last_ms;              /* device time of the unit's last launch; needs eri_plan_set_timing(plan,1)      */
   float last_ms_grad;
-  int32_t kernel_grad;        /* gradient kernel of the unit: 0 generic, 3 tile                  */
+  int32_t kernel_grad;        /* gradient kernel of the unit: 0 generic, 2 cooperative shared-memory, 3 tile */
   int32_t reserved_;
   double canonical_flops_grad;
 } eri_class_stat_t;
@@ -110,6 +116,16 @@ int eri_plan_set_timing(eri_plan_t* plan, int on);
 /* kernel selection: 0 = tuned kernels where one exists, tile family preferred (default), 1 = generic kernel everywhere
  * (reference path), 2 = tuned kernels without the tile family (register and cooperative families only) */
 int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode);
+/* Tuning knobs of the kernel selection (measured defaults); the kernels are re-selected like
+ * eri_plan_set_kernel_mode does.  The results do not depend on them beyond rounding (the test-suite uses them to run every
+ * kernel family on small inputs):
+ *   ERI_TUNE_TILE_FILL_SCALE  multiplies the lane-fill thresholds below which a unit is NOT given to the tile family
+ *                             (default 1; 0 = tile family wherever the class is served and the HRR guard passes)
+ *   ERI_TUNE_GRAD_MIN_TASKS   cooperative gradient kernel: the run of bra pairs per task (16) is halved while a unit has
+ *                             fewer tasks than this (default 32768; 0 = always runs of 16) */
+#define ERI_TUNE_TILE_FILL_SCALE 0
+#define ERI_TUNE_GRAD_MIN_TASKS 1
+int eri_plan_set_tuning(eri_plan_t* plan, int key, double value);
 /* Multi-GPU sharding: this process evaluates only the thread blocks b with b % nranks == rank of every
  * class launch (quartets are independent units).  The outputs are then PARTIAL sums; J, K and the gradient
  * are linear in them, so the caller sums the outputs over ranks (one all-reduce).  Default rank 0 of 1. */
@@ -148,6 +164,12 @@ int eri_c2s_matrix(int l, double* T /*HOST out*/);
 int eri_measure_fp64_peak(double* tflops /*HOST out*/, void* cuda_stream);
 /* Canonical FLOP count of one contracted quartet; deriv != 0: gradient count. */
 double eri_canonical_flops(int la, int lb, int lc, int ld, int ka, int kb, int kc, int kd, int deriv);
+
+/* Test diagnostics: the tuned kernel instantiations the library holds and those this process has launched so far, as
+ * newline-separated "family la lb lc ld" (family: reg, coop, tile, tgrad, cgrad; launched also: generic, generic_grad).
+ * Writes at most n bytes (NUL-terminated) to buf (HOST, may be NULL) and returns the size needed. */
+int eri_kernel_catalog(char* buf, int n);
+int eri_kernel_launched(char* buf, int n);
 
 const char* eri_strerror(int code);
 const char* eri_last_error(void);

@@ -11,6 +11,7 @@
 #include <memory>
 #include <mutex>
 #include <new>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -61,8 +62,12 @@ struct Dev {   // owning device array
 };
 
 // ---- process-wide read-only device data ---------------------------------------------------------------------
+// The library binds to the device that is current at its first compute call: the Rys buffer, the __constant__ c2s table and
+// the per-kernel shared-memory attributes live on that device.  Every later entry point checks that the same device is
+// current and fails with ERI_ERR_BAD_ARG otherwise (eri.h "Devices"); one process drives one GPU.
 std::mutex g_init_mu;
 double* g_rys = nullptr;
+int g_device = -1;
 bool g_c2s_ready = false;
 std::vector<double> g_c2s_host[LMAX + 1];
 
@@ -98,19 +103,32 @@ void build_c2s(int l, std::vector<double>& T) {
 
 int ensure_init() {
   std::lock_guard<std::mutex> lk(g_init_mu);
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (g_device >= 0 && dev != g_device)
+    return fail(ERI_ERR_BAD_ARG, "liberi_b200 is bound to CUDA device %d (current at its first call) but device %d is current", g_device, dev);
   if (!g_rys) {
     // consistency of the compile-time constants in eri_dev.cuh with the generated table
     for (int N = 1; N <= RYS_NMAX; ++N)
       if (rys_offset(N) != RYS_TABLE_OFFSET_H[N] || rys_xmax(N) != RYS_XMAX_H[N])
         return fail(ERI_ERR_BAD_ARG, "rys_tables.inc does not match eri_dev.cuh (N=%d)", N);
-    std::vector<double> h(RYS_HDR_SIZE + RYS_TABLE_SIZE, 0.0);
+    static_assert(RYS_TABLE_DOUBLES == RYS_TABLE_SIZE, "eri_dev.cuh: RYS_TABLE_DOUBLES must equal RYS_TABLE_SIZE of rys_tables.inc");
+    static_assert(RYS2_BASE % 2 == 0, "second table layout must start 16-byte aligned");
+    std::vector<double> h(RYS2_BASE + rys2_offset(RYS2_NMAX + 1), 0.0);
     for (int N = 1; N <= RYS_NMAX; ++N) { h[RYS_HDR_XMAX + N] = RYS_XMAX_H[N]; h[RYS_HDR_OFF + N] = RYS_TABLE_OFFSET_H[N]; }
     for (int k = 0; k < RYS_NMAX * (RYS_NMAX + 1) / 2; ++k) { h[RYS_HDR_H2 + k] = RYS_HERM_H2_H[k]; h[RYS_HDR_V + k] = RYS_HERM_V_H[k]; }
     std::memcpy(h.data() + RYS_HDR_SIZE, RYS_TABLE_H, sizeof(double) * RYS_TABLE_SIZE);
+    // second layout (eri_dev.cuh "Shared-memory copy"): [interval][value][k], padded interval stride
+    for (int N = 1; N <= RYS2_NMAX; ++N)
+      for (int iv = 0; iv < rys_nint(N); ++iv)
+        for (int k = 0; k < 14; ++k)
+          for (int n = 0; n < 2 * N; ++n)
+            h[RYS2_BASE + rys2_offset(N) + (size_t)iv * rys2_stride(N) + n * 14 + k] = RYS_TABLE_H[RYS_TABLE_OFFSET_H[N] + iv * (28 * N) + k * 2 * N + n];
     double* d = nullptr;
     CK(cudaMalloc(&d, h.size() * sizeof(double)));
     CK(cudaMemcpy(d, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice));
     g_rys = d;
+    g_device = dev;
   }
   if (!g_c2s_ready) {
     std::vector<double> all;
@@ -329,6 +347,8 @@ struct eri_plan {
   bool is_list = false, want_grad = false;
   double thr = 0.0;
   int kernel_mode = 0, timing = 0, shard = 0, nshard = 1, serial = 0;
+  double tile_fill_scale = 1.0;                       // eri_plan_set_tuning: multiplies the tile family's fill thresholds
+  long long grad_min_tasks = COOP_GRAD_MIN_TASKS;     // eri_plan_set_tuning: tasks per unit below which the cooperative gradient run is halved
   std::vector<std::unique_ptr<PairClass>> pcs;
   std::vector<std::unique_ptr<Unit>> units;
   Dev<int> sh_l, sh_sph, sh_cart, sph2sh, cart2sh;
@@ -409,7 +429,11 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
   TunedInfo ti{};
   u.kernel = 0; u.BI = GENERIC_BI; u.BJ = GENERIC_BJ;
   const bool canonical = P.la >= P.lb && R.la >= R.lb && (P.la > R.la || (P.la == R.la && P.lb >= R.lb));
-  if (pl.kernel_mode != 1 && canonical && tuned_jk_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel = ti.kind; u.BI = ti.BI; u.BJ = ti.BJ; }
+  if (pl.kernel_mode != 1 && canonical && tuned_jk_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) {
+    // the register family (kind 1) builds the 2-D integrals on the first centre of each pair like the tile family: same guard
+    // (the cooperative family chooses the centre per primitive pair; the generic kernel does too)
+    if (ti.kind != 1 || (P.hrr_loss <= HRR_LOSS_MAX && R.hrr_loss <= HRR_LOSS_MAX)) { u.kernel = ti.kind; u.BI = ti.BI; u.BJ = ti.BJ; }
+  }
   // tile family: dense mode, and only where building the 2-D integrals on the first centre of every pair is safe
   u.kernel_grad = 0; u.gBI = GENERIC_GRAD_BI; u.gBJ = GENERIC_GRAD_BJ;
   if (pl.kernel_mode == 0 && canonical && !pl.is_list && P.grouped && R.grouped) {
@@ -440,11 +464,12 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
     const double fill = u.t_slots > 0 ? (double)u.quartets / (double)u.t_slots : 0.0;
     if (P.hrr_loss <= HRR_LOSS_MAX && R.hrr_loss <= HRR_LOSS_MAX && tile_jk_info(P.la, P.lb, R.la, R.lb, &ti)) {
       // the register family (kind 1) is hard to beat on sparsely filled tiles; the cooperative family (kind 2) is not
-      const bool take = u.kernel == 1 ? (fill >= TILE_MIN_FILL && gb.fill >= TILE_MIN_BRA_FILL) : fill >= (ti.TQ >= 5 ? TILE_MIN_FILL : TILE_MIN_FILL_COOP);
+      const double fs = pl.tile_fill_scale;
+      const bool take = u.kernel == 1 ? (fill >= fs * TILE_MIN_FILL && gb.fill >= fs * TILE_MIN_BRA_FILL) : fill >= fs * (ti.TQ >= 5 ? TILE_MIN_FILL : TILE_MIN_FILL_COOP);
       if (take) { u.kernel = 3; u.tBI = ti.BI; }
     }
     // gradient: one more quantum is transferred (lb + 1, ld + 1 is not raised), so the loss bound is one power higher
-    if (pl.want_grad && fill >= TILE_MIN_FILL_GRAD && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
+    if (pl.want_grad && fill >= pl.tile_fill_scale * TILE_MIN_FILL_GRAD && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
         tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = 3; u.gBI = ti.BI; }
   }
   // cooperative gradient kernel for what the tile gradient kernel does not serve (it chooses the build centre itself)
@@ -452,7 +477,7 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
     u.kernel_grad = 2; u.gBI = ti.BI; u.gBJ = ti.BJ;
     // a warp walks its task's bra pairs one after the other: units of few, heavy quartets (the contracted core shells,
     // K^4 = 4096 primitive quartets each) get shorter runs so that they still spread over the SMs
-    while (u.gBI > 1 && u.quartets / u.gBI < COOP_GRAD_MIN_TASKS) u.gBI /= 2;
+    while (u.gBI > 1 && u.quartets / u.gBI < pl.grad_min_tasks) u.gBI /= 2;
   }
   if (!pl.is_list) {
     std::vector<int> ro;
@@ -491,9 +516,26 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
 constexpr int POOL_STREAMS = 8;
 constexpr long long POOL_BIG_BLOCKS = 4 * 148;   // at least four blocks per SM: the launch fills the GPU
 
+// which tuned instantiations this process has launched (eri_kernel_launched; read by the test-suite's coverage check)
+std::mutex g_log_mu;
+std::set<std::string> g_launched;
+void log_launch(const char* fam, const Work& w) {
+  char buf[64]; snprintf(buf, sizeof buf, "%s %d %d %d %d", fam, w.bra.la, w.bra.lb, w.ket.la, w.ket.lb);
+  std::lock_guard<std::mutex> lk(g_log_mu);
+  g_launched.insert(buf);
+}
+
 int launch_unit(eri_plan& pl, Unit& u, bool grad, double* gJ, double* gK, cudaStream_t s) {
   Work w = make_work(pl, u, grad);
   w.gJ = gJ; w.gK = gK;
+  {
+    const int k = grad ? u.kernel_grad : u.kernel;
+    TunedInfo ti{};
+    const char* fam = grad ? (k == 3 ? "tgrad" : k == 2 ? "cgrad" : "generic_grad")
+                           : (k == 3 ? "tile" : k == 2 ? "coop" : k == 1 ? "reg" : "generic");
+    (void)ti;
+    log_launch(fam, w);
+  }
   if (!grad) {
     if (u.kernel == 0) CK(launch_generic_jk(w, u.nblocks, s));
     else if (u.kernel == 3) CK(launch_tile_jk_class(w, u.t_nblocks, s));
@@ -692,7 +734,7 @@ int create_list_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* pr
     ctot += blk;
   }
   if (cart_total) *cart_total = ctot;
-  for (auto& pc : pl.pcs) CKI(upload_pair_class(b, *pc, s));
+  for (auto& pc : pl.pcs) { CKI(upload_pair_class(b, *pc, s)); pc->hrr_loss = hrr_loss_of(b, *pc, 0); pc->hrr_loss_grad = hrr_loss_of(b, *pc, 1); }
   for (size_t k = 0; k < pl.units.size(); ++k) {
     Unit& u = *pl.units[k];
     u.nlist = (int)lists[k].size(); u.quartets = u.nlist;
@@ -716,6 +758,7 @@ int create_list_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* pr
 
 int build_jk(eri_plan& pl, const double* D, double* J, double* K, cudaStream_t s) {
   if (!D || !J || !K) return fail(ERI_ERR_BAD_ARG, "null matrix pointer");
+  CKI(ensure_init());   // device check
   const size_t n2 = (size_t)pl.basis.nao_cart * pl.basis.nao_cart;
   if (pl.basis.nao == 0) return ERI_OK;
   CK(launch_sph2cart(pl.map, D, pl.Dc.p, s));
@@ -735,6 +778,7 @@ int build_jk(eri_plan& pl, const double* D, double* J, double* K, cudaStream_t s
 int jk_grad(eri_plan& pl, const double* D, double* gJ, double* gK, cudaStream_t s) {
   if (!D || !gJ || !gK) return fail(ERI_ERR_BAD_ARG, "null pointer");
   if (pl.is_list || !pl.want_grad) return fail(ERI_ERR_BAD_ARG, "plan was not created with want_grad");
+  CKI(ensure_init());   // device check
   if (pl.basis.natm == 0) return ERI_OK;
   CK(cudaMemsetAsync(gJ, 0, sizeof(double) * 3 * pl.basis.natm, s));
   CK(cudaMemsetAsync(gK, 0, sizeof(double) * 3 * pl.basis.natm, s));
@@ -874,11 +918,42 @@ int eri_plan_class_stats(const eri_plan_t* cplan, eri_class_stat_t* out, int max
   return k;
 }
 int eri_plan_set_timing(eri_plan_t* plan, int on) { if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan"); plan->timing = on; return ERI_OK; }
+static int reselect_kernels(eri_plan_t* plan) {
+  // the row tables of the new selection are uploaded on a private non-blocking stream and waited for here: host-synchronous
+  // like plan creation, but no device-wide synchronisation through the legacy default stream
+  cudaStream_t st = nullptr;
+  CK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+  int rc = ERI_OK;
+  for (auto& u : plan->units) { rc = select_kernels(*plan, *u, st); if (rc != ERI_OK) break; }
+  cudaStreamSynchronize(st); cudaStreamDestroy(st);
+  plan->order.clear(); plan->order_grad.clear();
+  return rc;
+}
 int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode) {
   if (!plan || mode < 0 || mode > 2) return fail(ERI_ERR_BAD_ARG, "bad kernel mode");
+  CKI(ensure_init());   // device check
   plan->kernel_mode = mode;
-  for (auto& u : plan->units) CKI(select_kernels(*plan, *u, nullptr));
-  return ERI_OK;
+  return reselect_kernels(plan);
+}
+int eri_plan_set_tuning(eri_plan_t* plan, int key, double value) {
+  if (!plan || !(value >= 0.0)) return fail(ERI_ERR_BAD_ARG, "bad tuning value");
+  CKI(ensure_init());
+  if (key == ERI_TUNE_TILE_FILL_SCALE) plan->tile_fill_scale = value;
+  else if (key == ERI_TUNE_GRAD_MIN_TASKS) plan->grad_min_tasks = (long long)value;
+  else return fail(ERI_ERR_BAD_ARG, "unknown tuning key %d", key);
+  return reselect_kernels(plan);
+}
+int eri_kernel_catalog(char* buf, int n) {
+  std::vector<std::string> v; tuned_catalog(v);
+  std::string all; for (const std::string& x : v) { all += x; all += '\n'; }
+  if (buf && n > 0) { const size_t m = std::min((size_t)n - 1, all.size()); std::memcpy(buf, all.data(), m); buf[m] = 0; }
+  return (int)all.size() + 1;
+}
+int eri_kernel_launched(char* buf, int n) {
+  std::string all;
+  { std::lock_guard<std::mutex> lk(g_log_mu); for (const std::string& x : g_launched) { all += x; all += '\n'; } }
+  if (buf && n > 0) { const size_t m = std::min((size_t)n - 1, all.size()); std::memcpy(buf, all.data(), m); buf[m] = 0; }
+  return (int)all.size() + 1;
 }
 
 int eri_build_jk(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim, const double* coords, int natm,
@@ -980,12 +1055,13 @@ int eri_c2s_matrix(int l, double* T) {   // diagnostic: the library's ns(l) x nc
 
 int eri_measure_fp64_peak(double* tflops, void* stream) {
   if (!tflops) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  CKI(ensure_init());   // device check
   cudaStream_t s = (cudaStream_t)stream;
   int dev = 0, sms = 0;
   CK(cudaGetDevice(&dev)); CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   Dev<double> sink; CK(sink.alloc(1));
   cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
-  const int blocks = sms * 8, iters = 20000;
+  const int blocks = sms * 8, iters = 100000;   // at least 1e5 iterations
   CK(launch_fp64_peak(sink.p, 2000, blocks, s));
   double best = 0.0;
   for (int rep = 0; rep < 5; ++rep) {

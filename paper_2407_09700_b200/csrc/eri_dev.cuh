@@ -66,6 +66,64 @@ template <int N>
 __device__ __forceinline__ void rys_roots(double x, const double* __restrict__ rys, double* u, double* w) {
   rys_roots_impl<int>(N, rys_offset(N), rys_xmax(N), x, rys, u, w);
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Shared-memory copy of one N's Chebyshev table for the thread-per-quartet families (tile, register, tile gradient).
+// There every lane has its own x, hence its own interval: read from global memory, the 28 N coefficient loads of a
+// primitive quartet touch up to 32 different 128-byte lines each and the L1/TEX data pipe, not the FP64 pipe, bounds
+// the low-l classes (profiles/r02_cfg3.md: 75 % of its peak, 7 sectors per request).  The second layout
+//   [interval][value n = 0..2N-1 (u_0.., w_0..)][k = 0..13]
+// keeps the 14 coefficients of a value contiguous, so a lane fetches them with seven 128-bit shared loads; lanes in the
+// same interval read the same address (broadcast); the interval stride is padded to 2 (mod 16) doubles, i.e. to 1 (mod 8)
+// 16-byte slots, so that different intervals fall into different slots of a 128-byte wavefront.
+// The buffer holds the layout after the first one, at RYS2_BASE (16-byte aligned).
+constexpr int RYS_TABLE_DOUBLES = 34636;                       // = RYS_TABLE_SIZE of rys_tables.inc (checked in api.cu)
+constexpr int RYS2_BASE = RYS_HDR_SIZE + RYS_TABLE_DOUBLES;    // even: 16-byte aligned
+constexpr int RYS2_NMAX = 6;                                   // classes of the thread-per-quartet families have N <= 6
+__host__ __device__ constexpr int rys2_stride(int N) { int s = 28 * N; while (s % 16 != 2) ++s; return s; }
+__host__ __device__ constexpr int rys2_size(int N) { return rys_nint(N) * rys2_stride(N); }
+__host__ __device__ constexpr int rys2_offset(int N) { int off = 0; for (int n = 1; n < N; ++n) off += rys2_size(n); return off; }
+
+// all threads of the block: copy the class's table to shared memory (dst 16-byte aligned); the caller synchronises
+template <int N>
+__device__ __forceinline__ void rys_stage_table(double* __restrict__ dst, const double* __restrict__ rys, int tid, int nthreads) {
+  static_assert(N <= RYS2_NMAX, "no second-layout table for this N");
+  const double2* src = reinterpret_cast<const double2*>(rys + RYS2_BASE + rys2_offset(N));
+  double2* d = reinterpret_cast<double2*>(dst);
+  for (int i = tid; i < rys2_size(N) / 2; i += nthreads) d[i] = src[i];
+}
+
+// same rule, same arithmetic and summation order as rys_roots_impl (bit-identical results), coefficients from `tab`
+template <int N>
+__device__ __forceinline__ void rys_roots_smem(double x, const double* __restrict__ tab, const double* __restrict__ rys, double* u, double* w) {
+  if (x >= rys_xmax(N)) {
+    const double rx = 1.0 / x, rs = sqrt(rx);
+    const double* h2 = rys + RYS_HDR_H2 + N * (N - 1) / 2;
+    const double* v = rys + RYS_HDR_V + N * (N - 1) / 2;
+#pragma unroll
+    for (int n = 0; n < N; ++n) { u[n] = h2[n] * rx; w[n] = v[n] * rs; }
+    return;
+  }
+  const int iv = (int)(x * 0.4);
+  const double s = (x - (2.5 * iv + 1.25)) * 0.8, s2 = 2.0 * s;
+  const double2* c = reinterpret_cast<const double2*>(tab + iv * rys2_stride(N));
+#pragma unroll
+  for (int n = 0; n < 2 * N; ++n) {
+    const double2 p6 = c[n * 7 + 6];
+    double b1 = p6.y, b2 = 0.0;
+    double t = fma(s2, b1, p6.x - b2); b2 = b1; b1 = t;           // k = 12
+#pragma unroll
+    for (int j = 5; j >= 1; --j) {
+      const double2 pj = c[n * 7 + j];
+      t = fma(s2, b1, pj.y - b2); b2 = b1; b1 = t;                // k = 2j + 1
+      t = fma(s2, b1, pj.x - b2); b2 = b1; b1 = t;                // k = 2j
+    }
+    const double2 p0 = c[n * 7];
+    t = fma(s2, b1, p0.y - b2); b2 = b1; b1 = t;                  // k = 1
+    const double val = fma(s, b1, p0.x - b2);
+    if (n < N) u[n] = val; else w[n - N] = val;
+  }
+}
 __device__ inline void rys_roots_rt(int N, double x, const double* __restrict__ rys, double* u, double* w) {
   rys_roots_impl<int>(N, (int)rys[RYS_HDR_OFF + N], rys[RYS_HDR_XMAX + N], x, rys, u, w);
 }

@@ -1,6 +1,8 @@
 // launch.h -- host-callable launchers of the kernel translation units of liberi_b200 (internal, not part of the ABI).
 #pragma once
 #include <cuda_runtime.h>
+#include <string>
+#include <vector>
 #include "eri_dev.cuh"
 
 namespace eri {
@@ -25,6 +27,8 @@ cudaError_t launch_tuned_grad(const Work& w, int nblocks_dense, cudaStream_t s);
 // cooperative gradient kernel (kind 2, dense mode): info->BI x info->BJ = bra pairs per task x ket pairs per block
 bool coop_grad_info(int la, int lb, int lc, int ld, TunedInfo* info);
 cudaError_t launch_coop_grad_class(const Work& w, int nblocks_dense, cudaStream_t s);
+
+void tuned_catalog(std::vector<std::string>& out);   // "family la lb lc ld" of every tuned instantiation
 
 // transform.cu
 cudaError_t upload_c2s(const double* tables /*host, concatenated ns(l) x nc(l), l = 0..4*/);

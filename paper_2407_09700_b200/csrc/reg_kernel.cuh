@@ -71,6 +71,9 @@ __global__ void __launch_bounds__(REG_BJ * REG_BI) reg_jk_kernel(Work w) {
   constexpr int G2 = (LA + 1) * (LB + 1) * (LC + 1) * (LD + 1);
   constexpr int SB = (LC + 1) * (LD + 1), SA = (LB + 1) * SB, SC = LD + 1;
   __shared__ double red[NCD * REG_BI * REG_BJ];
+  extern __shared__ __align__(16) double rtab[];   // Rys table of the class (eri_dev.cuh "Shared-memory copy"), dynamic shared memory
+  rys_stage_table<N>(rtab, w.rys, threadIdx.y * REG_BJ + threadIdx.x, REG_BJ * REG_BI);
+  __syncthreads();
 
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
@@ -118,7 +121,7 @@ __global__ void __launch_bounds__(REG_BJ * REG_BI) reg_jk_kernel(Work w) {
         const double pref = Kab * Kcd * sqrt(rpq);
         const double hq = 0.5 / q;
         double u[N], wt[N];
-        rys_roots<N>(x, w.rys, u, wt);
+        rys_roots_smem<N>(x, rtab, w.rys, u, wt);
 #pragma unroll
         for (int r = 0; r < N; ++r) {
           const double t2 = u[r] * rpq;          // u / (p+q)
@@ -284,7 +287,8 @@ cudaError_t launch_reg_jk(const Work& w, int nblocks_dense, cudaStream_t s) {
   const int total = w.list ? (w.nlist + REG_BJ * REG_BI - 1) / (REG_BJ * REG_BI) : nblocks_dense;
   const int grid = (total + w.nshard - 1) / w.nshard;
   if (grid <= 0) return cudaSuccess;
-  reg_jk_kernel<LA, LB, LC, LD><<<grid, dim3(REG_BJ, REG_BI), 0, s>>>(w);
+  constexpr size_t rt_bytes = sizeof(double) * rys2_size(nroots_of(LA + LB + LC + LD));   // < 48 KB with the static part: no attribute needed
+  reg_jk_kernel<LA, LB, LC, LD><<<grid, dim3(REG_BJ, REG_BI), rt_bytes, s>>>(w);
   return cudaGetLastError();
 }
 

@@ -23,7 +23,8 @@ struct TileGradTraits {
   static constexpr int NLANE = NC * ND + NA * ND + NB * ND;                       // D_cd, D_ad, D_bd: per lane
   static constexpr int STAGE = 32 * 33;
   static constexpr int PERWARP = STAGE + NUNI + 32 * NLANE;
-  static constexpr size_t SMEM = sizeof(double) * BI * PERWARP;
+  static constexpr int RT = rys2_size(N);                    // the class's Rys table, first in the block's shared memory
+  static constexpr size_t SMEM = sizeof(double) * (RT + BI * PERWARP);
 };
 
 // One differentiated axis AX of one root (MODE 1): the 2-D integrals of axis AX are built raised on A, B, C, those of the
@@ -95,7 +96,7 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
   using Tr = TileGradTraits<LA, LB, LC, LD, BI>;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, N = Tr::N, G2 = Tr::G2;
   constexpr int SD = 1, SC = LD + 1, SB = (LC + 2) * SC, SA = (LB + 2) * SB;   // strides of the raised 2-D arrays
-  extern __shared__ double smem[];
+  extern __shared__ __align__(16) double smem[];
 
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
@@ -103,7 +104,10 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
   const int r = find_row_warp(w.row_off, w.nrows, blk, threadIdx.x);
   const int x = threadIdx.x, gq = threadIdx.y;
   const int i_first = w.row_slot[r], j_first = (blk - w.row_off[r]) * 32;
-  double* stage = smem + gq * Tr::PERWARP;
+  const double* rtab = smem;                       // Rys table of the class (eri_dev.cuh "Shared-memory copy")
+  rys_stage_table<N>(smem, w.rys, gq * 32 + x, 32 * BI);
+  __syncthreads();
+  double* stage = smem + Tr::RT + gq * Tr::PERWARP;
   double* uni = stage + Tr::STAGE;                 // [D_ab | D_ac | D_bc], the same for all lanes
   double* mine = uni + Tr::NUNI + x;               // column of this lane, stride 32: [D_cd | D_ad | D_bd]
   const int half = x >> 4;                         // ket half of this lane: its own shell c
@@ -182,7 +186,7 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
           const double pref = f * Kab * Kcd * sqrt(rpq);
           const double hq = 0.5 / q;
           double u[N], wt[N];
-          rys_roots<N>(xx, w.rys, u, wt);
+          rys_roots_smem<N>(xx, rtab, w.rys, u, wt);
           if constexpr (MODE == 1) {
 #pragma unroll 1
             for (int rt = 0; rt < N; ++rt) {

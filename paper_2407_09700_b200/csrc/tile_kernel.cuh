@@ -191,7 +191,8 @@ struct TileTraits {
   static constexpr int MINB = (NT == 128 && RW <= 63) ? 3 : (NT == 256 && TQ == 1 && RW >= 30) ? 2 : (NT == 256 && RW <= 15) ? 4 : 0;
   static constexpr int NKEEP = NCD + NAT * ND;              // per-thread sums kept over the rows: J_cd, K_ad
   static constexpr int STAGE = max3(reduce_stage_size(NABT), reduce_stage_size(NAT * NC), reduce_stage_size(NB * NC));   // doubles per warp
-  static constexpr size_t SMEM = sizeof(double) * (NW * STAGE + NKEEP * NT);
+  static constexpr int RT = rys2_size(N);                    // the class's Rys table, first in the block's shared memory (16-byte aligned)
+  static constexpr size_t SMEM = sizeof(double) * (RT + NW * STAGE + NKEEP * NT);
 };
 
 template <int LA, int LB, int LC, int LD, int TQ, int BI>
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
   using Tr = TileTraits<LA, LB, LC, LD, TQ, BI>;
   constexpr int NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAT = Tr::NAT, NABT = Tr::NABT, NCD = Tr::NCD, NE = Tr::NE;
   constexpr int N = Tr::N, G2 = Tr::G2, NT = Tr::NT, NKEEP = Tr::NKEEP;
-  extern __shared__ double smem[];
+  extern __shared__ __align__(16) double smem[];
 
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
@@ -207,10 +208,13 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
   const int r = find_row_warp(w.row_off, w.nrows, blk, threadIdx.x);
   const int x = threadIdx.x, wy = threadIdx.y, gq = wy / TQ, t = wy - gq * TQ, tid = wy * 32 + x;
   const int i_first = w.row_slot[r], j_first = (blk - w.row_off[r]) * 32;
-  double* stage = smem + wy * Tr::STAGE;
-  double* keep = smem + Tr::NW * Tr::STAGE + tid;   // keep[e * NT]: [0, NCD) J_cd ; [NCD, NCD + NAT*ND) K_ad
+  const double* rtab = smem;                        // Rys table of the class (eri_dev.cuh "Shared-memory copy")
+  rys_stage_table<N>(smem, w.rys, tid, NT);
+  double* stage = smem + Tr::RT + wy * Tr::STAGE;
+  double* keep = smem + Tr::RT + Tr::NW * Tr::STAGE + tid;   // keep[e * NT]: [0, NCD) J_cd ; [NCD, NCD + NAT*ND) K_ad
 #pragma unroll
   for (int e = 0; e < NKEEP; ++e) keep[e * NT] = 0.0;
+  __syncthreads();
 
   // ---- this lane's ket pair (fixed for the whole block) ----
   const int j = j_first + x;
@@ -264,7 +268,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
           const double pref = f * Kab * Kcd * sqrt(rpq);
           const double hq = 0.5 / q;
           double u[N], wt[N];
-          rys_roots<N>(xx, w.rys, u, wt);
+          rys_roots_smem<N>(xx, rtab, w.rys, u, wt);
 #pragma unroll
           for (int rt = 0; rt < N; ++rt) {
             const double t2 = u[rt] * rpq;
@@ -401,7 +405,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
 
   // ---- block end: J_cd summed over all warps, K_ad over the warps of the same team member; one atomic per element ----
   __syncthreads();
-  const double* kall = smem + Tr::NW * Tr::STAGE;
+  const double* kall = smem + Tr::RT + Tr::NW * Tr::STAGE;
   for (int o = tid; o < NCD * 32; o += NT) {
     const int e = o >> 5, lane = o & 31;
     double sum = 0.0;

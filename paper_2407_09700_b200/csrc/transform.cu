@@ -134,6 +134,23 @@ __global__ void rys_diag_kernel(int N, const double* __restrict__ rys, const dou
   for (int k = 0; k < N; ++k) { u[(long)t * N + k] = uu[k]; w[(long)t * N + k] = ww[k]; }
 }
 
+// N <= RYS2_NMAX: the same points through the shared-memory copy of the table (rys_roots_smem, used by the thread-per-quartet
+// families); the two routes share coefficients and summation order, so any bit of difference is reported as NaN
+template <int N>
+__global__ void rys_diag_smem_kernel(const double* __restrict__ rys, const double* __restrict__ x, int n,
+                                     double* __restrict__ u, double* __restrict__ w) {
+  extern __shared__ __align__(16) double tab[];
+  rys_stage_table<N>(tab, rys, threadIdx.x, blockDim.x);
+  __syncthreads();
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  double uu[N], ww[N], u2[9], w2[9];
+  rys_roots_smem<N>(x[t], tab, rys, uu, ww);
+  rys_roots_rt(N, x[t], rys, u2, w2);
+  const double bad = __longlong_as_double(0x7ff8000000000000LL);
+  for (int k = 0; k < N; ++k) { u[(long)t * N + k] = uu[k] == u2[k] ? uu[k] : bad; w[(long)t * N + k] = ww[k] == w2[k] ? ww[k] : bad; }
+}
+
 // 16 independent FMA chains per thread; 2 flops per FMA
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double* sink, int iters) {
   double a[16];
@@ -183,7 +200,14 @@ cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, doubl
 
 cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, double* u, double* w, cudaStream_t s) {
   if (n <= 0) return cudaSuccess;
-  rys_diag_kernel<<<(n + 127) / 128, 128, 0, s>>>(N, rys, x, n, u, w);
+  const int grid = (n + 127) / 128;
+  switch (N) {
+#define CASE(NN) case NN: rys_diag_smem_kernel<NN><<<grid, 128, sizeof(double) * rys2_size(NN), s>>>(rys, x, n, u, w); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6)
+#undef CASE
+    default: rys_diag_kernel<<<grid, 128, 0, s>>>(N, rys, x, n, u, w);
+  }
+  static_assert(RYS2_NMAX == 6, "launch_rys_diag lists the second-layout tables up to N = 6");
   return cudaGetLastError();
 }
 

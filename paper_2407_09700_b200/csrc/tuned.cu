@@ -1,4 +1,7 @@
 // tuned.cu -- dispatch table of the per-class tuned kernels: register family (reg_g*.cu), cooperative family (coop_*.cu).
+#include <cstdio>
+#include <string>
+#include <vector>
 #include "launch.h"
 #include "reg_classes.h"
 #include "coop_classes.h"
@@ -137,6 +140,28 @@ cudaError_t launch_tuned_grad(const Work& w, int nblocks, cudaStream_t s) {
   TRY(0) TRY(1) TRY(2) TRY(3) TRY(4) TRY(5) TRY(6) TRY(7)
 #undef TRY
   return cudaErrorNotSupported;
+}
+
+// every (family, class) instantiation the library holds, "family la lb lc ld" (eri_kernel_catalog)
+void tuned_catalog(std::vector<std::string>& out) {
+  auto add = [&](const char* fam, int a, int b, int c, int d) {
+    char buf[64]; snprintf(buf, sizeof buf, "%s %d %d %d %d", fam, a, b, c, d); out.push_back(buf);
+  };
+#define X(a, b, c, d) add("reg", a, b, c, d);
+  REG_GROUP0(X) REG_GROUP1(X) REG_GROUP2(X) REG_GROUP3(X)
+#undef X
+#define X(a, b, c, d, tw, nch) add("coop", a, b, c, d);
+  COOP_ALL(X)
+#undef X
+#define X(a, b, c, d, tq, bi) add("tile", a, b, c, d);
+  TILE_ALL(X)
+#undef X
+#define X(a, b, c, d, bi, mode) add("tgrad", a, b, c, d);
+  TGRAD_ALL(X)
+#undef X
+#define X(a, b, c, d, wp, em) add("cgrad", a, b, c, d);
+  CGRAD_ALL(X)
+#undef X
 }
 
 }  // namespace eri

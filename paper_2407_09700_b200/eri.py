@@ -39,7 +39,8 @@ class eri_class_stat_t(ctypes.Structure):
 
 EXPORTS = ["eri_build_jk", "eri_jk_grad", "eri_plan_create", "eri_plan_build_jk", "eri_plan_jk_grad",
            "eri_plan_build_jk_host", "eri_plan_jk_grad_host", "eri_plan_stats", "eri_plan_num_classes",
-           "eri_plan_class_stats", "eri_plan_set_timing", "eri_plan_set_kernel_mode", "eri_plan_set_shard", "eri_plan_destroy",
+           "eri_plan_class_stats", "eri_plan_set_timing", "eri_plan_set_kernel_mode", "eri_plan_set_tuning", "eri_plan_set_shard", "eri_plan_destroy",
+           "eri_kernel_catalog", "eri_kernel_launched",
            "eri_compute_quartets", "eri_digest_quartet_list", "eri_list_plan_create", "eri_list_plan_digest",
            "eri_schwarz", "eri_rys_roots", "eri_c2s_matrix", "eri_measure_fp64_peak", "eri_canonical_flops",
            "eri_strerror", "eri_last_error", "eri_version"]
@@ -70,6 +71,9 @@ def lib():
         L.eri_plan_set_timing.argtypes = [_vp, ctypes.c_int]
         L.eri_plan_set_kernel_mode.argtypes = [_vp, ctypes.c_int]
         L.eri_plan_set_shard.argtypes = [_vp, ctypes.c_int, ctypes.c_int]
+        L.eri_plan_set_tuning.argtypes = [_vp, ctypes.c_int, _f64]
+        L.eri_kernel_catalog.argtypes = [ctypes.c_char_p, ctypes.c_int]
+        L.eri_kernel_launched.argtypes = [ctypes.c_char_p, ctypes.c_int]
         _lib_handle = L
     return _lib_handle
 
@@ -170,6 +174,9 @@ class Plan:
     def set_kernel_mode(self, mode: int):
         _check(lib().eri_plan_set_kernel_mode(self._h, int(mode)))
 
+    def set_tuning(self, key: int, value: float):
+        _check(lib().eri_plan_set_tuning(self._h, int(key), float(value)))
+
     def set_shard(self, rank: int, nranks: int):
         _check(lib().eri_plan_set_shard(self._h, int(rank), int(nranks)))
 
@@ -269,6 +276,26 @@ def eri_measure_fp64_peak() -> float:
 
 def eri_canonical_flops(la, lb, lc, ld, ka, kb, kc, kd, deriv=False) -> float:
     return float(lib().eri_canonical_flops(la, lb, lc, ld, ka, kb, kc, kd, int(bool(deriv))))
+
+
+ERI_TUNE_TILE_FILL_SCALE, ERI_TUNE_GRAD_MIN_TASKS = 0, 1
+
+
+def _string_list(fn) -> list[str]:
+    n = fn(None, 0)
+    buf = ctypes.create_string_buffer(n)
+    fn(buf, n)
+    return [x for x in buf.value.decode().split("\n") if x]
+
+
+def eri_kernel_catalog() -> list[str]:
+    """every tuned kernel instantiation of the library, 'family la lb lc ld'"""
+    return _string_list(lib().eri_kernel_catalog)
+
+
+def eri_kernel_launched() -> list[str]:
+    """the instantiations this process has launched so far"""
+    return _string_list(lib().eri_kernel_launched)
 
 
 def eri_version() -> str:

@@ -206,6 +206,40 @@ def cfg4():
     return b, D, 1e-13
 
 
+# ----------------------------------------------------------------------------- chain workload
+def _basis_spd(rng, scale):
+    """Polarised split-valence-like heavy atom: s(K=6) core, s(3)+s(1) and p(3)+p(1) valence, one d; seeded synthetic
+    even-tempered exponents, `scale` separates the element kinds (no real basis-set data)."""
+    return [_even_tempered(rng, 0, 6, 9.0 * scale, 3.1), _even_tempered(rng, 0, 3, 0.9 * scale, 3.3), _even_tempered(rng, 0, 1, 0.22 * scale, 1.0),
+            _even_tempered(rng, 1, 3, 0.9 * scale, 3.4), _even_tempered(rng, 1, 1, 0.2 * scale, 1.0),
+            _even_tempered(rng, 2, 1, 0.8, 1.0)]
+
+
+def chain(n_res: int = 30, seed: int = SEED0 + 5, thr: float = 1e-10):
+    """Long, spatially extended system with the shapes of the paper's polyglycine set (Table I: Gly_30 with
+    a polarised double-zeta basis has 213 atoms and 1878 functions): a zigzag chain of n_res residues of 4 heavy atoms
+    (N, C, C, O kinds) and 3 hydrogens, 3.63 A per residue, terminated by H and OH; heavy atoms 3s2p1d (core s contracted
+    over 6 primitives), hydrogen 2s; spherical functions.  Here screening decides the time (tau = 1e-10 as in the paper).
+    The geometry and all basis-set numbers are synthetic stand-ins: the paper's test set is not in this container."""
+    rng = np.random.default_rng(seed)
+    tmpl = [("N", (0.00, 0.30, 0.0)), ("H", (0.00, 1.30, 0.0)), ("C", (1.21, -0.45, 0.0)), ("H", (1.21, -1.10, 0.88)),
+            ("H", (1.21, -1.10, -0.88)), ("C", (2.42, 0.35, 0.0)), ("O", (2.42, 1.58, 0.0))]
+    kinds, xyz = [], []
+    for i in range(n_res):
+        sgn = 1.0 if i % 2 == 0 else -1.0
+        for k, (x, y, z) in tmpl:
+            kinds.append(k); xyz.append((3.63 * i + x, sgn * y, z))
+    sgn = 1.0 if (n_res - 1) % 2 == 0 else -1.0
+    kinds += ["H", "O", "H"]
+    xyz += [(-0.90, -0.15, 0.0), (3.63 * (n_res - 1) + 3.60, -sgn * 0.35, 0.0), (3.63 * (n_res - 1) + 4.15, sgn * 0.45, 0.0)]
+    xyz = (np.array(xyz) + rng.normal(0.0, 0.03, (len(xyz), 3))) * ANGSTROM
+    shells = {"C": _basis_spd(rng, 1.0), "N": _basis_spd(rng, 1.35), "O": _basis_spd(rng, 1.75),
+              "H": [_even_tempered(rng, 0, 3, 0.45, 4.2), _even_tempered(rng, 0, 1, 0.16, 1.0)]}
+    basis = _assemble([shells[k] for k in kinds], xyz, {"name": f"chain{n_res}", "n_res": n_res, "basis": "spd", "seed": seed})
+    D = _density_cct(rng, basis.nao, 15 * n_res + 5)
+    return basis, D, thr
+
+
 # ----------------------------------------------------------------------------- cfg1: ERI class microbenchmark
 def canonical_classes(lmax: int = 4) -> list[tuple[int, int, int, int]]:
     """(la,lb,lc,ld) with la>=lb, lc>=ld, (la,lb)>=(lc,ld); 120 classes for lmax=4."""

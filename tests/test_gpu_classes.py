@@ -14,8 +14,10 @@ torch = pytest.importorskip("torch")
 from paper_2407_09700_b200 import workloads as W  # noqa: E402
 
 CLASSES_F = [c for c in W.canonical_classes(4) if max(c) <= 3]
-CLASSES_G = [(4, 0, 0, 0), (4, 1, 1, 0), (4, 0, 2, 0), (4, 2, 2, 1), (4, 3, 1, 0), (4, 4, 2, 0), (4, 1, 4, 1), (4, 4, 3, 2), (4, 3, 4, 3),
-             (4, 3, 3, 3), (4, 4, 4, 2), (4, 4, 4, 4), (4, 4, 3, 3), (4, 4, 4, 3)]   # the last six: ket components of shell c in chunks (coop_kernel.cuh, NCH > 1)
+CLASSES_G = [c for c in W.canonical_classes(4) if max(c) == 4]   # all 65 g classes: every cooperative instantiation (TW, NCH, PASSES differ per class)
+# contraction degrees 1 and 3 beside 2 (BASELINE.json configs[1]: K in {1, 3, 6}; K = 6 in test_gpu_parity.CFG1_CASES) on classes of every family
+CLASSES_K13 = [(0, 0, 0, 0), (1, 0, 1, 0), (2, 1, 1, 0), (1, 1, 1, 1), (2, 1, 2, 1), (2, 2, 2, 0), (3, 1, 2, 1), (3, 3, 1, 0), (3, 2, 3, 2),
+               (4, 0, 1, 0), (4, 1, 4, 0), (4, 4, 0, 0), (4, 2, 3, 1)]
 
 
 @pytest.fixture(scope="module")
@@ -31,14 +33,17 @@ def _n_for(cls):
     size = 1
     for l in cls:
         size *= (l + 1) * (l + 2) // 2
-    return 64 if size <= 100 else 24 if size <= 2000 else 8
+    return 64 if size <= 100 else 24 if size <= 2000 else 8 if size <= 12000 else 5
 
 
-@pytest.mark.parametrize("cls", CLASSES_F + CLASSES_G, ids=lambda c: "".join("spdfg"[l] for l in c))
-def test_class_list_digest(eri, orc, cls):
-    assert len(CLASSES_F) == 55
+CASES = [(c, 2) for c in CLASSES_F + CLASSES_G] + [(c, k) for c in CLASSES_K13 for k in (1, 3)]
+
+
+@pytest.mark.parametrize("cls,K", CASES, ids=lambda v: "".join("spdfg"[l] for l in v) if isinstance(v, tuple) else f"K{v}")
+def test_class_list_digest(eri, orc, cls, K):
+    assert len(CLASSES_F) == 55 and len(CLASSES_G) == 65
     n = _n_for(cls)
-    basis, D, q = W.cfg1_class(cls, 2, nquartets=n, pool=6)
+    basis, D, q = W.cfg1_class(cls, K, nquartets=n, pool=6)
     Dd = torch.from_numpy(D).cuda()
     Jo, Ko = orc.digest_list(basis, D, q)
     scale = max(np.abs(Jo).max(), np.abs(Ko).max(), 1e-300)

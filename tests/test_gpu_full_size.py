@@ -76,10 +76,10 @@ def test_cfg3_sampled_blocks_against_oracle(eri, orc, cfg3_jk):
     scale = np.abs(J).max()
     assert np.abs(J - J.T).max() <= 1e-13 * scale and np.abs(K - K.T).max() <= 1e-13 * scale
     assert np.isfinite(J).all() and np.isfinite(K).all()
-    pj = _sample_pairs(basis, 2407, 1)
+    pj = _sample_pairs(basis, 2407, 6)     # 6 per (l_i, l_j) combination + 3 core-shell pairs = 63 blocks (64 + 64)
     for (i, j), blk in zip(pj, orc.j_blocks(basis, D, pj)):
         assert np.abs(_block(J, basis, i, j) - blk).max() <= JK_TOL * scale, ("J", i, j)
-    pk = _sample_pairs(basis, 9700, 1)
+    pk = _sample_pairs(basis, 9700, 6)
     for (i, j), blk in zip(pk, orc.k_blocks(basis, D, pk)):
         assert np.abs(_block(K, basis, i, j) - blk).max() <= JK_TOL * scale, ("K", i, j)
 
@@ -127,6 +127,43 @@ def test_cfg4_gradient_sum_rule_and_finite_differences(eri):
         fdJ, fdK = (e[0][0] - e[1][0]) / (2 * h), (e[0][1] - e[1][1]) / (2 * h)
         # truncation error of the central difference ~ h^2 f''' / 6 and rounding ~ 1e-16 E / h with E ~ 1e3
         assert abs(fdJ - gJ[atom, ax]) <= 2e-6 and abs(fdK - gK[atom, ax]) <= 2e-6, (atom, ax, fdJ, gJ[atom, ax], fdK, gK[atom, ax])
+
+
+def test_cfg4_full_size_gradient_row_against_oracle(eri, orc):
+    """SURVEY 8(c) cfg4 procedure at full size, in bench.py's launch configuration: the oracle's row mode (all quartets with
+    the differentiated function on the atom, same Schwarz screening) for one hydrogen of the 16-water cluster; that row of
+    the GPU gradient must match to BASELINE.json's 1e-8 Hartree/Bohr.  Covers what only large units reach: the runs of
+    2..16 bra pairs per task of the cooperative gradient kernel and the re-routed (x|ps), (dp|ps) units."""
+    basis, D, thr = W.cfg4()
+    plan = eri.eri_plan_create(basis, thr, want_grad=True)
+    gJ, gK = plan.jk_grad(dev(D))
+    gJ, gK = gJ.cpu().numpy(), gK.cpu().numpy()
+    atom = 3 * 9 + 1                                               # first H of the tenth molecule (inside the cluster)
+    rJ, rK = orc.jk_grad(basis, D, atoms=[atom], thr=thr)
+    assert np.abs(gJ[atom] - rJ[atom]).max() <= GRAD_TOL, (gJ[atom], rJ[atom])
+    assert np.abs(gK[atom] - rK[atom]).max() <= GRAD_TOL, (gK[atom], rK[atom])
+    # the three kernel selections agree on the whole gradient (generic = mode 1 is the reference path)
+    for mode in (2, 1):
+        plan.set_kernel_mode(mode)
+        hJ, hK = plan.jk_grad(dev(D))
+        assert np.abs(hJ.cpu().numpy() - gJ).max() <= GRAD_TOL and np.abs(hK.cpu().numpy() - gK).max() <= GRAD_TOL, mode
+
+
+def test_gradient_four_water_tz_against_oracle(eri, orc):
+    """full oracle gradient of a 4-water cluster with the cfg4 basis (88 shells), default kernel selection and
+    the cooperative kernel forced to full runs of 16 bra pairs (the multi-bra-pair path under the oracle)."""
+    basis, D = W.water_cluster((1, 2, 2), "tz", 43, "tz4g")
+    gJo, gKo = orc.jk_grad(basis, D, thr=1e-13)
+    plan = eri.eri_plan_create(basis, 1e-13, want_grad=True)
+    for tasks in (None, 0.0):
+        if tasks is not None:
+            plan.set_tuning(eri.ERI_TUNE_GRAD_MIN_TASKS, tasks)
+        gJ, gK = plan.jk_grad(dev(D))
+        assert np.abs(gJ.cpu().numpy() - gJo).max() <= GRAD_TOL, tasks
+        assert np.abs(gK.cpu().numpy() - gKo).max() <= GRAD_TOL, tasks
+    plan.set_kernel_mode(2)                                        # no tile family: everything on the cooperative gradient kernel, runs of 16
+    gJ, gK = plan.jk_grad(dev(D))
+    assert np.abs(gJ.cpu().numpy() - gJo).max() <= GRAD_TOL and np.abs(gK.cpu().numpy() - gKo).max() <= GRAD_TOL
 
 
 def test_gradient_two_water_tz_against_oracle(eri, orc):
