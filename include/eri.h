@@ -102,6 +102,18 @@ int eri_plan_build_jk(eri_plan_t* plan, const double* D /*DEVICE*/, double* J /*
                       void* cuda_stream);
 int eri_plan_jk_grad(eri_plan_t* plan, const double* D /*DEVICE*/, double* grad_J /*DEVICE*/, double* grad_K /*DEVICE*/,
                      void* cuda_stream);
+/* Density-weighted batch screening of the paper (Eq. 8-9 and Algorithm 1 lines 12-16), the step that makes
+ * repeated SCF iterations cheap: J and K of D as eri_plan_build_jk, but a unique quartet of the unit
+ * {ab|cd} (shell groups a, b, c, d: equal angular momentum and contraction degree) is evaluated iff
+ *     Q_ij * Q_kl * min(1, P_{ab|cd}) >= schwarz_thr,   P_{ab|cd} = max |D| over the six sub-blocks of D between the groups,
+ * computed per call from D on the device (no host synchronisation).  The cap at 1 keeps the kept set inside the plan's
+ * Schwarz-only list.  Linear in D like the plain build, so an incremental Fock build calls it with D_new - D_old, whose
+ * small elements remove most of the list.  The error against the unscreened result is bounded like the Schwarz rule's:
+ * each skipped quartet contributes less than schwarz_thr per matrix element.  D, J, K DEVICE.  schwarz_thr = 0: same as
+ * eri_plan_build_jk.  eri_plan_dscreen_quartets: unique quartets evaluated by the last such call (waits for it). */
+int eri_plan_build_jk_dscreen(eri_plan_t* plan, const double* D /*DEVICE*/, double* J /*DEVICE*/, double* K /*DEVICE*/,
+                              void* cuda_stream);
+int eri_plan_dscreen_quartets(eri_plan_t* plan, int64_t* out /*HOST*/);
 /* Same work with HOST buffers: H2D copy of D, build, D2H copy of the results, stream synchronised on return. */
 int eri_plan_build_jk_host(eri_plan_t* plan, const double* D /*HOST*/, double* J /*HOST*/, double* K /*HOST*/,
                            void* cuda_stream);

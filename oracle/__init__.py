@@ -44,6 +44,7 @@ def lib():
         _lib = ctypes.CDLL(build())
         _lib.oracle_prim_eri.restype = ctypes.c_double
         _lib.oracle_jk.restype = ctypes.c_longlong
+        _lib.oracle_jk_dscreen.restype = ctypes.c_longlong
         for l in range(5):
             T = sph.c2s(l)
             _lib.oracle_set_c2s(l, _d(T))
@@ -111,6 +112,23 @@ def jk(basis, D, thr: float = 0.0):
     K = np.zeros_like(D)
     args, keep = _basis_args(basis)
     n = lib().oracle_jk(*args, _d(D), ctypes.c_double(thr), _d(J), _d(K))
+    return J, K, int(n)
+
+
+def shell_groups(basis) -> np.ndarray:
+    """Group id of every shell: shells of equal (l, nprim) form a set |a, K_a}; ids in sorted (l, K) order."""
+    keys = sorted({(int(s["l"]), int(s["nprim"])) for s in basis.shells})
+    return np.array([keys.index((int(s["l"]), int(s["nprim"]))) for s in basis.shells], dtype=np.int32)
+
+
+def jk_dscreen(basis, D, thr: float):
+    """J, K with the density-weighted batch screening of Eq. 8-9 at the level of shell groups; see md_oracle.cpp."""
+    D = np.ascontiguousarray(D, dtype=np.float64)
+    J = np.zeros_like(D)
+    K = np.zeros_like(D)
+    g = shell_groups(basis)
+    args, keep = _basis_args(basis)
+    n = lib().oracle_jk_dscreen(*args, _d(D), ctypes.c_double(thr), _i(g), ctypes.c_int(int(g.max()) + 1), _d(J), _d(K))
     return J, K, int(n)
 
 

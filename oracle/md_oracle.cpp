@@ -426,12 +426,34 @@ void oracle_schwarz(const int32_t* shells, int nsh, const double* prims, int npr
 // J_ij = sum_kl (ij|kl) D_kl,  K_ik = sum_jl (ij|kl) D_jl : plain loop over ALL ordered shell quartets.
 // thr > 0: "same screening" mode, skips exactly the quartets with Q_ij Q_kl < thr (reading R7), Q from this oracle.
 // Returns the number of shell quartets evaluated.
-long long oracle_jk(const int32_t* shells, int nsh, const double* prims, int npr, const double* xyz, int natm,
-                    const double* D, double thr, double* J, double* K) {
+// group_of != nullptr: density-weighted screening of the paper (Eq. 8-9) at the level of shell groups:
+// a quartet is skipped iff Q_ij Q_kl min(1, P) < thr with P = max |D| over the six sub-blocks of D between the shell groups
+// of i, j, k, l (the groups are the caller's: shells of equal angular momentum and contraction degree).
+// The cap at 1 makes the density factor only ever remove quartets from the Schwarz-only list.
+static long long jk_loop(const int32_t* shells, int nsh, const double* prims, int npr, const double* xyz, int natm,
+                         const double* D, double thr, const int32_t* group_of, int ng, double* J, double* K) {
   BasisView bv = view(shells, nsh, prims, npr, xyz, natm);
   const int nao = bv.nao;
   PairTable pt; pt.build(bv);
   std::vector<double> Q; if (thr > 0) schwarz_matrix(bv, pt, Q);
+  std::vector<double> Pg;   // Pg[ga][gb] = max |D_mu,nu|, mu in a shell of group ga, nu in a shell of group gb
+  if (group_of) {
+    Pg.assign((size_t)ng * ng, 0.0);
+    for (int a = 0; a < nsh; ++a)
+      for (int b = 0; b < nsh; ++b)
+        for (int m = 0; m < nsph(bv.sh[a].l); ++m)
+          for (int n = 0; n < nsph(bv.sh[b].l); ++n) {
+            double& p = Pg[(size_t)group_of[a] * ng + group_of[b]];
+            p = std::max(p, std::fabs(D[(size_t)(bv.sh[a].ao_off + m) * nao + bv.sh[b].ao_off + n]));
+          }
+  }
+  auto dens_factor = [&](int i, int j, int k, int l) {
+    if (!group_of) return 1.0;
+    const int g[4] = {group_of[i], group_of[j], group_of[k], group_of[l]};
+    double P = 0.0;
+    for (int x = 0; x < 4; ++x) for (int y = 0; y < 4; ++y) if (x != y) P = std::max(P, Pg[(size_t)g[x] * ng + g[y]]);
+    return std::min(1.0, P);
+  };
   std::fill(J, J + (size_t)nao * nao, 0.0); std::fill(K, K + (size_t)nao * nao, 0.0);
   long long count = 0;
 #pragma omp parallel reduction(+ : count)
@@ -444,7 +466,7 @@ long long oracle_jk(const int32_t* shells, int nsh, const double* prims, int npr
       const int ni = nsph(si.l), nj = nsph(sj.l);
       for (int k = 0; k < nsh; ++k)
         for (int l = 0; l < nsh; ++l) {
-          if (thr > 0 && Q[(size_t)i * nsh + j] * Q[(size_t)k * nsh + l] < thr) continue;
+          if (thr > 0 && Q[(size_t)i * nsh + j] * Q[(size_t)k * nsh + l] * dens_factor(i, j, k, l) < thr) continue;
           const Shell& sk = bv.sh[k]; const Shell& sl = bv.sh[l];
           const int nk = nsph(sk.l), nl = nsph(sl.l);
           blk.resize((size_t)ni * nj * nk * nl);
@@ -464,6 +486,16 @@ long long oracle_jk(const int32_t* shells, int nsh, const double* prims, int npr
     for (size_t x = 0; x < (size_t)nao * nao; ++x) K[x] += Kp[x];
   }
   return count;
+}
+
+long long oracle_jk(const int32_t* shells, int nsh, const double* prims, int npr, const double* xyz, int natm,
+                    const double* D, double thr, double* J, double* K) {
+  return jk_loop(shells, nsh, prims, npr, xyz, natm, D, thr, nullptr, 0, J, K);
+}
+
+long long oracle_jk_dscreen(const int32_t* shells, int nsh, const double* prims, int npr, const double* xyz, int natm,
+                            const double* D, double thr, const int32_t* group_of, int ng, double* J, double* K) {
+  return jk_loop(shells, nsh, prims, npr, xyz, natm, D, thr, group_of, ng, J, K);
 }
 
 // Block mode for large systems: Jblk for shell pairs (i,j) = sum over all (k,l); Kblk for shell pairs (i,k) = sum over all (j,l).

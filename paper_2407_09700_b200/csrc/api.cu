@@ -331,7 +331,9 @@ struct Unit {
   double flops = 0, flops_grad = 0;
   float last_ms = 0, last_ms_grad = 0;
   std::vector<int> h_count;
+  int index = 0;                            // position in eri_plan::units
   Dev<int> ket_count, row_off, g_row_off;
+  Dev<int> ket_count_dyn;                   // density-weighted call: kept prefix per bra pair under tau / P_{ab|cd}
   Dev<int> t_row_slot, t_row_off; int t_nrows = 0, t_nblocks = 0, tBI = 0; long long t_slots = 0;   // tile family
   Dev<int2> list; int nlist = 0;            // list mode
   Dev<long long> coff;                      // list mode, store kernel
@@ -353,6 +355,10 @@ struct eri_plan {
   std::vector<std::unique_ptr<Unit>> units;
   Dev<int> sh_l, sh_sph, sh_cart, sph2sh, cart2sh;
   Dev<double> Dc, Jc, Kc, Dh, Jh, Kh, gJd, gKd;   // Cartesian workspaces; device staging for the *_host entry points
+  // density-weighted screening (eri_plan_build_jk_dscreen): AO -> shell group, group sub-block maxima of |D|, per unit the
+  // effective threshold and the number of quartets that passed in the last call
+  Dev<int> ao_group; Dev<unsigned long long> pmax, ds_kept; Dev<double> thr_eff; Dev<DscreenUnit> ds_units;
+  int ds_max_nbra = 0; bool ds_ready = false, ds_active = false;
   ShellMap map{};
   eri_stats_t stats{};
   std::vector<cudaEvent_t> ev;   // timing mode: ev[k] before unit k, ev[n] after the last one (no host sync in between)
@@ -498,6 +504,7 @@ Work make_work(const eri_plan& pl, const Unit& u, bool grad) {
   Work w{};
   w.bra = pl.pcs[u.P]->view(); w.ket = pl.pcs[u.R]->view();
   w.ket_count = u.ket_count.p;
+  if (pl.ds_active && !grad) { w.ket_count = u.ket_count_dyn.p; w.thr_dev = pl.thr_eff.p + u.index; }
   w.row_off = grad ? u.g_row_off.p : u.row_off.p;
   w.nrows = grad ? u.g_nrows : u.nrows;
   w.thr = pl.thr;
@@ -674,6 +681,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
       CK(u->ket_count.upload(u->h_count, s));
       CKI(select_kernels(pl, *u, s));
       qkept += tot; flops += u->flops; flops_g += u->flops_grad;
+      u->index = (int)pl.units.size();
       pl.units.push_back(std::move(u));
     }
   CK(cudaStreamSynchronize(s));
@@ -775,6 +783,38 @@ int build_jk(eri_plan& pl, const double* D, double* J, double* K, cudaStream_t s
   return ERI_OK;
 }
 
+// Density-weighted batch screening (Eq. 8-9 and Alg. 1 lines 12-16): per call, from the density itself,
+// P_{ab|cd} = the largest |D| over the six sub-blocks between the four shell groups of a unit; a quartet of the unit is
+// evaluated iff Q_ij Q_kl min(1, P_{ab|cd}) >= tau.  All of it runs on the device on the caller's stream (no host
+// synchronisation): one pass over D, then one launch that writes each unit's effective threshold, the kept ket prefix
+// of every bra pair and the number of surviving quartets.
+int dscreen_prepare(eri_plan& pl, const double* D, cudaStream_t s) {
+  const Basis& b = pl.basis;
+  const int ng = (int)b.groups.size(), nu = (int)pl.units.size();
+  if (!pl.ds_ready) {
+    std::vector<int> ag(b.nao);
+    for (size_t sh = 0; sh < b.sh.size(); ++sh)
+      for (int k = 0; k < nsph(b.sh[sh].l); ++k) ag[b.sh[sh].ao_off + k] = b.group_of[sh];
+    CK(pl.ao_group.upload(ag, s));
+    CK(pl.pmax.alloc((size_t)ng * ng)); CK(pl.ds_kept.alloc(nu)); CK(pl.thr_eff.alloc(nu));
+    std::vector<DscreenUnit> du(nu);
+    for (int k = 0; k < nu; ++k) {
+      Unit& u = *pl.units[k]; const PairClass& P = *pl.pcs[u.P]; const PairClass& R = *pl.pcs[u.R];
+      CK(u.ket_count_dyn.alloc(P.npair));
+      du[k] = DscreenUnit{P.q.p, R.q.p, u.ket_count.p, u.ket_count_dyn.p, P.npair, {P.ga, P.gb, R.ga, R.gb}};
+      pl.ds_max_nbra = std::max(pl.ds_max_nbra, P.npair);
+    }
+    CK(pl.ds_units.upload(du, s));
+    CK(cudaStreamSynchronize(s));   // the host vectors die here (first call only)
+    pl.ds_ready = true;
+  }
+  CK(cudaMemsetAsync(pl.pmax.p, 0, sizeof(unsigned long long) * ng * ng, s));
+  CK(cudaMemsetAsync(pl.ds_kept.p, 0, sizeof(unsigned long long) * nu, s));
+  CK(launch_group_max(D, b.nao, pl.ao_group.p, ng, pl.pmax.p, s));
+  CK(launch_dscreen(pl.ds_units.p, nu, pl.ds_max_nbra, pl.pmax.p, ng, pl.thr, pl.thr_eff.p, pl.ds_kept.p, s));
+  return ERI_OK;
+}
+
 int jk_grad(eri_plan& pl, const double* D, double* gJ, double* gK, cudaStream_t s) {
   if (!D || !gJ || !gK) return fail(ERI_ERR_BAD_ARG, "null pointer");
   if (pl.is_list || !pl.want_grad) return fail(ERI_ERR_BAD_ARG, "plan was not created with want_grad");
@@ -856,6 +896,28 @@ int eri_list_plan_digest(eri_plan_t* plan, const double* D, double* Jt, double* 
 int eri_plan_jk_grad(eri_plan_t* plan, const double* D, double* gJ, double* gK, void* stream) {
   if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan");
   return jk_grad(*plan, D, gJ, gK, (cudaStream_t)stream);
+}
+
+int eri_plan_build_jk_dscreen(eri_plan_t* plan, const double* D, double* J, double* K, void* stream) {
+  if (!plan || !D || !J || !K) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  if (plan->is_list) return fail(ERI_ERR_BAD_ARG, "list plan: density-weighted screening needs a dense plan");
+  if (!(plan->thr > 0.0)) return eri_plan_build_jk(plan, D, J, K, stream);   // tau = 0: nothing is ever skipped
+  CKI(ensure_init());
+  if (plan->basis.nao == 0) return ERI_OK;
+  CKI(dscreen_prepare(*plan, D, (cudaStream_t)stream));
+  plan->ds_active = true;
+  const int rc = build_jk(*plan, D, J, K, (cudaStream_t)stream);
+  plan->ds_active = false;
+  return rc;
+}
+int eri_plan_dscreen_quartets(eri_plan_t* plan, int64_t* out) {
+  if (!plan || !out) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  *out = 0;
+  if (!plan->ds_ready) return ERI_OK;
+  std::vector<unsigned long long> h(plan->units.size());
+  CK(cudaMemcpy(h.data(), plan->ds_kept.p, sizeof(unsigned long long) * h.size(), cudaMemcpyDeviceToHost));
+  for (unsigned long long v : h) *out += (int64_t)v;
+  return ERI_OK;
 }
 
 int eri_plan_build_jk_host(eri_plan_t* plan, const double* D, double* J, double* K, void* stream) {

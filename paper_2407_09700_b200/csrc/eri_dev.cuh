@@ -173,6 +173,9 @@ struct Work {
   const int* row_slot;
   double thr;
   int grad_ch;       // cooperative gradient kernel: bra pairs per task (Unit::gBI)
+  // density-weighted screening (Eq. 8-9; eri_plan_build_jk_dscreen): the unit's effective threshold
+  // tau / P_{ab|cd} in device memory (tile family; the other families get a per-call ket_count); nullptr: use thr
+  const double* thr_dev;
 };
 
 __device__ __forceinline__ void atomic_add(double* p, double v) { atomicAdd(p, v); }

@@ -45,6 +45,12 @@ cudaError_t launch_block_c2s(const ShellMap& m, const int* q4, int n, const doub
                              double* out, const long long* ooff, cudaStream_t s);
 // Q[t] = sqrt(max_{s,t'} |(s t'|s t')|) over spherical components from the Cartesian block (ab|ab) [nab][nab] at cart + t*nab*nab
 cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, double* Q, cudaStream_t s);
+// density-weighted screening (transform.cu): shell-group sub-block maxima of |D|, then per unit the effective threshold,
+// the per-call kept ket counts and the number of quartets that pass
+struct DscreenUnit { const double* qb; const double* qk; const int* count; int* count_dyn; int nbra; int g[4]; };
+cudaError_t launch_group_max(const double* D, int nao, const int* ao_group, int ng, unsigned long long* pmax, cudaStream_t s);
+cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, const unsigned long long* pmax, int ng, double tau,
+                           double* thr_eff, unsigned long long* kept, cudaStream_t s);
 cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, double* u, double* w, cudaStream_t s);
 cudaError_t launch_fp64_peak(double* sink, int iters, int blocks, cudaStream_t s);
 

@@ -229,13 +229,14 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
   const double* __restrict__ D = w.D;
   double* __restrict__ Jm = w.J; double* __restrict__ Km = w.K;
   int a0 = -1;                         // first Cartesian AO of shell a owned by this thread
+  const double thr = w.thr_dev ? *w.thr_dev : w.thr;   // density-weighted call: tau / P_{ab|cd} of this unit (Eq. 8-9)
 
 #pragma unroll 1
   for (int y = gq; y < TILE_ROWS; y += BI) {
     const int i = i_first + y;
     const double qi = bp.q[i];
-    if (qi < 0.0 || qi * qk_max < w.thr) break;            // rows are sorted: no later row has work (reading R7)
-    const bool active = qj >= 0.0 && qi * qj >= w.thr && (!w.same || j <= i);
+    if (qi < 0.0 || qi * qk_max < thr) break;              // rows are sorted: no later row has work (reading R7)
+    const bool active = qj >= 0.0 && qi * qj >= thr && (!w.same || j <= i);
     if (!__any_sync(0xffffffffu, active)) continue;
     const int2 ab0 = bp.ao[i];
     a0 = ab0.x + t * NAT;

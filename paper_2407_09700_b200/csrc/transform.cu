@@ -151,6 +151,47 @@ __global__ void rys_diag_smem_kernel(const double* __restrict__ rys, const doubl
   for (int k = 0; k < N; ++k) { u[(long)t * N + k] = uu[k] == u2[k] ? uu[k] : bad; w[(long)t * N + k] = ww[k] == w2[k] ? ww[k] : bad; }
 }
 
+// ---- density-weighted screening (Eq. 8-9) -------------------------------------------------------------
+// P_{a|b} = max |D| over the sub-block of the (spherical) density between shell groups a and b: one pass over D.
+__global__ void group_max_kernel(const double* __restrict__ D, int nao, const int* __restrict__ ao_group, int ng,
+                                 unsigned long long* __restrict__ pmax) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long)nao * nao) return;
+  const int i = (int)(t / nao), j = (int)(t - (long)i * nao);
+  const double v = fabs(D[t]);
+  if (v > 0.0) atomicMax(pmax + ao_group[i] * ng + ao_group[j], (unsigned long long)__double_as_longlong(v));   // non-negative doubles order like integers
+}
+
+// per unit u: thr_eff[u] = tau / P_{ab|cd}, P = the largest of the six group sub-block maxima (Eq. 9); per bra pair i the
+// kept kets are the prefix of the Schwarz-sorted ket set with q_i q_j >= thr_eff (Alg. 1 lines 12-16 in the limit of fine
+// bins), never more than the plan's Schwarz-only count; kept[u] = number of quartets of the unit that pass.
+__global__ void dscreen_kernel(const DscreenUnit* __restrict__ units, const unsigned long long* __restrict__ pmax, int ng, double tau,
+                               double* __restrict__ thr_eff, unsigned long long* __restrict__ kept) {
+  const DscreenUnit U = units[blockIdx.y];
+  const int g[4] = {U.g[0], U.g[1], U.g[2], U.g[3]};
+  double P = 0.0;
+#pragma unroll
+  for (int x = 0; x < 4; ++x)
+#pragma unroll
+    for (int y = 0; y < 4; ++y)
+      if (x != y) P = fmax(P, __longlong_as_double((long long)pmax[g[x] * ng + g[y]]));
+  const double te = P > 0.0 ? tau / P : 1.0e300;
+  if (blockIdx.x == 0 && threadIdx.x == 0) thr_eff[blockIdx.y] = te;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int cnt = 0;
+  if (i < U.nbra) {
+    const double qi = U.qb[i];
+    int lo = 0, hi = U.count[i];                 // largest prefix with q_i q_j >= thr_eff (q sorted descending)
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (qi * U.qk[mid] >= te) lo = mid + 1; else hi = mid; }
+    cnt = lo;
+    U.count_dyn[i] = cnt;
+  }
+  unsigned long long c = cnt;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+  if ((threadIdx.x & 31) == 0 && c) atomicAdd(kept + blockIdx.y, c);
+}
+
 // 16 independent FMA chains per thread; 2 flops per FMA
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double* sink, int iters) {
   double a[16];
@@ -208,6 +249,20 @@ cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, do
     default: rys_diag_kernel<<<grid, 128, 0, s>>>(N, rys, x, n, u, w);
   }
   static_assert(RYS2_NMAX == 6, "launch_rys_diag lists the second-layout tables up to N = 6");
+  return cudaGetLastError();
+}
+
+cudaError_t launch_group_max(const double* D, int nao, const int* ao_group, int ng, unsigned long long* pmax, cudaStream_t s) {
+  const long n2 = (long)nao * nao;
+  if (n2 == 0) return cudaSuccess;
+  group_max_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, s>>>(D, nao, ao_group, ng, pmax);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, const unsigned long long* pmax, int ng, double tau,
+                           double* thr_eff, unsigned long long* kept, cudaStream_t s) {
+  if (nunits == 0) return cudaSuccess;
+  dscreen_kernel<<<dim3((max_nbra + 127) / 128, nunits), 128, 0, s>>>(units, pmax, ng, tau, thr_eff, kept);
   return cudaGetLastError();
 }
 

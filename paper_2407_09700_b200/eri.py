@@ -38,7 +38,7 @@ class eri_class_stat_t(ctypes.Structure):
 
 
 EXPORTS = ["eri_build_jk", "eri_jk_grad", "eri_plan_create", "eri_plan_build_jk", "eri_plan_jk_grad",
-           "eri_plan_build_jk_host", "eri_plan_jk_grad_host", "eri_plan_stats", "eri_plan_num_classes",
+           "eri_plan_build_jk_dscreen", "eri_plan_dscreen_quartets", "eri_plan_build_jk_host", "eri_plan_jk_grad_host", "eri_plan_stats", "eri_plan_num_classes",
            "eri_plan_class_stats", "eri_plan_set_timing", "eri_plan_set_kernel_mode", "eri_plan_set_tuning", "eri_plan_set_shard", "eri_plan_destroy",
            "eri_kernel_catalog", "eri_kernel_launched",
            "eri_compute_quartets", "eri_digest_quartet_list", "eri_list_plan_create", "eri_list_plan_digest",
@@ -62,7 +62,8 @@ def lib():
         L.eri_canonical_flops.restype = _f64
         L.eri_plan_destroy.restype = None
         L.eri_plan_destroy.argtypes = [_vp]
-        for name in ("eri_plan_build_jk", "eri_plan_jk_grad", "eri_plan_build_jk_host", "eri_plan_jk_grad_host",
+        L.eri_plan_dscreen_quartets.argtypes = [_vp, ctypes.POINTER(_i64)]
+        for name in ("eri_plan_build_jk", "eri_plan_build_jk_dscreen", "eri_plan_jk_grad", "eri_plan_build_jk_host", "eri_plan_jk_grad_host",
                      "eri_list_plan_digest"):
             getattr(L, name).argtypes = [_vp, _vp, _vp, _vp, _vp]
         L.eri_plan_stats.argtypes = [_vp, ctypes.POINTER(eri_stats_t)]
@@ -132,6 +133,20 @@ class Plan:
         fn = lib().eri_list_plan_digest if self.is_list else lib().eri_plan_build_jk
         _check(fn(self._h, _dev_f64(D, (n, n)), _dev_f64(J, (n, n)), _dev_f64(K, (n, n)), _stream()))
         return J, K
+
+    def build_jk_dens(self, D, J=None, K=None):
+        """eri_plan_build_jk_dscreen: the build with the density factor of Eq. 8-9 in the screening test"""
+        import torch
+        n = self.basis.nao
+        J = torch.empty((n, n), dtype=torch.float64, device=D.device) if J is None else J
+        K = torch.empty((n, n), dtype=torch.float64, device=D.device) if K is None else K
+        _check(lib().eri_plan_build_jk_dscreen(self._h, _dev_f64(D, (n, n)), _dev_f64(J, (n, n)), _dev_f64(K, (n, n)), _stream()))
+        return J, K
+
+    def dens_quartets(self) -> int:
+        v = _i64(0)
+        _check(lib().eri_plan_dscreen_quartets(self._h, ctypes.byref(v)))
+        return int(v.value)
 
     def jk_grad(self, D, gJ=None, gK=None):
         import torch

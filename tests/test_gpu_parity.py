@@ -175,6 +175,37 @@ def test_screening_equals_oracle_same_screening(eri, orc):
     assert st["quartets_kept"] < st["quartets_total"]
 
 
+def test_density_weighted_screening_equals_oracle_rule(eri, orc):
+    """SURVEY 8(f) NEXT-1 (Eq. 8-9, Alg. 1 lines 12-16): eri_plan_build_jk_dscreen evaluates exactly the quartets
+    with Q_ij Q_kl min(1, P_{ab|cd}) >= tau, P from the density itself; the oracle's jk_dscreen applies the same rule to its
+    plain quadruple loop.  A small "delta-D" (an SCF-like density change) removes most of the list."""
+    basis, D = W.water_cluster((1, 2, 2), "dzp", 31, "dzp4")
+    thr = 1e-6
+    plan = eri.eri_plan_create(basis, thr)
+    nk = plan.stats()["quartets_kept"]
+    rng = np.random.default_rng(12)
+    G = rng.standard_normal(D.shape)
+    for name, M in (("D", D), ("deltaD", 1e-3 * np.abs(D).max() * 0.5 * (G + G.T))):
+        for mode in (0, 2, 1):                                      # tile + register + cooperative, no tile family, generic
+            plan.set_kernel_mode(mode)
+            J, K = plan.build_jk_dens(dev(M))
+            kept = plan.dens_quartets()
+            Jo, Ko, _ = orc.jk_dscreen(basis, M, thr)
+            scale = np.abs(Jo).max()
+            assert np.abs(J.cpu().numpy() - Jo).max() <= 1e-9 * scale, (name, mode)   # pairs within rounding of the threshold may differ
+            assert np.abs(K.cpu().numpy() - Ko).max() <= 1e-9 * scale, (name, mode)
+            assert 0 < kept <= nk
+            if name == "deltaD":
+                assert kept < 0.7 * nk, (kept, nk)                 # the density factor did remove work
+                Ju, Ku, _ = orc.jk(basis, M, 0.0)                   # and the result is still the J/K of delta-D within the screening error
+                assert np.abs(J.cpu().numpy() - Ju).max() <= 1e-3 * np.abs(Ju).max()
+    plan.set_kernel_mode(0)
+    # the plain build is unchanged by the density-weighted calls before it
+    J, K = plan.build_jk(dev(D))
+    Jo, Ko, _ = orc.jk(basis, D, thr)
+    assert np.abs(J.cpu().numpy() - Jo).max() <= 1e-9 * np.abs(Jo).max()
+
+
 # ----------------------------------------------------------------------------------------------- cfg1 lists
 CFG1_CASES = [((0, 0, 0, 0), 1, 256), ((1, 0, 0, 0), 3, 256), ((1, 1, 1, 1), 3, 128), ((2, 1, 1, 1), 1, 128),
               ((2, 2, 2, 2), 1, 64), ((3, 3, 3, 3), 1, 16), ((3, 2, 1, 0), 6, 32), ((4, 4, 3, 3), 1, 8), ((4, 4, 4, 4), 1, 4),
@@ -225,7 +256,15 @@ def test_grad_mixed_up_to_g(eri, orc):
     basis = mixed_basis(seed=15, K=1, lmax=4, ncentre=2)
     rng = np.random.default_rng(4)
     C = rng.standard_normal((basis.nao, 6)) / math.sqrt(basis.nao)
-    _grad_parity(eri, orc, basis, C @ C.T, 0.0)
+    D = C @ C.T
+    _grad_parity(eri, orc, basis, D, 0.0)
+    # kernel mode 2 (no tile family): every class that has a cooperative gradient kernel runs on it, all 120 classes occur here
+    plan = eri.eri_plan_create(basis, 0.0, want_grad=True)
+    plan.set_kernel_mode(2)
+    assert {c["kernel_grad"] for c in plan.class_stats()} <= {0, 2}
+    gJ, gK = plan.jk_grad(dev(D))
+    gJo, gKo = orc.jk_grad(basis, D)
+    assert np.abs(gJ.cpu().numpy() - gJo).max() <= GRAD_TOL and np.abs(gK.cpu().numpy() - gKo).max() <= GRAD_TOL
 
 
 def test_grad_finite_difference_of_gpu_energy(eri):

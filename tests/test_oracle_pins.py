@@ -397,6 +397,43 @@ def test_block_modes_and_list_digest(orc, tiny):
     assert np.allclose(Kt, Kr, atol=1e-13 * max(np.abs(Jr).max(), 1e-3))
 
 
+def test_density_weighted_screening_mode_is_the_rule_written_out(orc):
+    """oracle.jk_dscreen (Eq. 8-9, PAPER.md:78-89 at shell-group level) == the oracle's own blocks summed over exactly the
+    quartets with Q_ij Q_kl min(1, P) >= tau, the rule evaluated here in numpy; a scaled-down density removes quartets."""
+    b, D, _ = W.cfg0()
+    D = 1e-3 * D
+    thr = 1e-3
+    n, nao = b.nshell, b.nao
+    off, dim = b.shells["ao_off"], 2 * b.shells["l"] + 1
+    g = orc.shell_groups(b)
+    assert list(g) == [0 if l == 0 else 1 for l in b.shells["l"]]
+    Q = orc.schwarz(b)
+    ng = g.max() + 1
+    Pg = np.zeros((ng, ng))
+    for i in range(n):
+        for j in range(n):
+            Pg[g[i], g[j]] = max(Pg[g[i], g[j]], np.abs(D[off[i]:off[i] + dim[i], off[j]:off[j] + dim[j]]).max())
+    J, K = np.zeros_like(D), np.zeros_like(D)
+    kept = 0
+    for i in range(n):
+        for j in range(n):
+            for k in range(n):
+                for l in range(n):
+                    gs = [g[i], g[j], g[k], g[l]]
+                    P = min(1.0, max(Pg[gs[x], gs[y]] for x in range(4) for y in range(4) if x != y))
+                    if Q[i, j] * Q[k, l] * P < thr:
+                        continue
+                    kept += 1
+                    blk = orc.eri_block(b, i, j, k, l)
+                    si, sj, sk, sl = [slice(off[x], off[x] + dim[x]) for x in (i, j, k, l)]
+                    J[si, sj] += np.einsum("abcd,cd->ab", blk, D[sk, sl])
+                    K[si, sk] += np.einsum("abcd,bd->ac", blk, D[sj, sl])
+    Jd, Kd, nd = orc.jk_dscreen(b, D, thr)
+    _, _, ns = orc.jk(b, D, thr)
+    assert nd == kept and kept < ns < n ** 4
+    assert np.allclose(Jd, J, atol=1e-14 * np.abs(J).max()) and np.allclose(Kd, K, atol=1e-14 * np.abs(J).max())
+
+
 # ------------------------------------------------------------------------------------------------ gradient
 def test_eri_derivative_block_vs_finite_difference(orc):
     b, D, _ = W.cfg0()
