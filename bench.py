@@ -537,7 +537,8 @@ def main():
     line = {"metric": METRIC, "value": nq / (ms * 1e-3), "unit": "quartets/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": desc, "nao": nao, "nshell": basis.nshell, "quartets_kept": nq, "quartets_total": st["quartets_total"],
-                       "pairs_kept": st["pairs_kept"], "canonical_flops": flops, "plan_ms": st["plan_ms"], "oneshot_ms": oneshot_ms,
+                       "pairs_kept": st["pairs_kept"], "canonical_flops": flops, "plan_ms": st["plan_ms"],
+                       "plan_ms_parts": {k: st["plan_ms_" + k] for k in ("init", "schwarz", "pairs", "units")}, "oneshot_ms": oneshot_ms,
                        "l2": "flushed between timed steps (256 MB fill)", "kernel_mode": args.kernel_mode,
                        "parallelism": f"replicated plan, thread blocks dealt round-robin over {world} ranks, NCCL all-reduce of J,K" if world > 1 else "single GPU"},
             "jk_build_ms_per_call": ms, "canonical_tflops": flops / (ms * 1e-3) / 1e12, "fp64_peak_measured_tflops": fp64_peak,

@@ -68,6 +68,8 @@ typedef struct {
   double canonical_flops;     /* DESIGN.md "FLOP model" summed over kept quartets (energy)    */
   double canonical_flops_grad;
   double plan_ms;             /* host wall time of eri_plan_create                            */
+  double plan_ms_init, plan_ms_schwarz, plan_ms_pairs, plan_ms_units;   /* its parts: basis + tables; pair sets + Schwarz factors;
+                                                                           prescreen, sort, grouped twins; work units + kernel selection */
 } eri_stats_t;
 
 /* One (bra pair class, ket pair class) work unit = one kernel launch. */

@@ -615,6 +615,8 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
   pl.thr = thr; pl.want_grad = want_grad != 0;
   const Basis& b = pl.basis;
   const int ng = (int)b.groups.size();
+  auto lap = [&, last = t0]() mutable { const auto now = std::chrono::steady_clock::now(); const double ms = std::chrono::duration<double, std::milli>(now - last).count(); last = now; return ms; };
+  pl.stats.plan_ms_init = lap();
   // pair sets |ab, KaKb} for group(a) >= group(b) (groups sorted by (l,K), so la >= lb) -- Alg. 1 lines 3-6
   std::vector<std::unique_ptr<PairClass>> all;
   double qmax = 0.0;
@@ -634,6 +636,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
       for (double q : pc->Q) qmax = std::max(qmax, q);
       all.push_back(std::move(pc));
     }
+  pl.stats.plan_ms_schwarz = lap();
   // prescreen (Alg. 1 line 7), sort by decreasing bound (the paper bins, Eq. 6; sorting is the limit of fine bins)
   long long pairs_kept = 0;
   for (auto& pc : all) {
@@ -655,6 +658,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
   std::sort(pl.pcs.begin(), pl.pcs.end(), [](const std::unique_ptr<PairClass>& x, const std::unique_ptr<PairClass>& y) {
     return std::make_tuple(x->la, x->lb, x->ga, x->gb) < std::make_tuple(y->la, y->lb, y->ga, y->gb);
   });
+  pl.stats.plan_ms_pairs = lap();
   // work units: bra set P >= ket set R; per bra pair the kept kets are a prefix of the sorted ket set (reading R7)
   long long qkept = 0; double flops = 0, flops_g = 0;
   for (int P = 0; P < (int)pl.pcs.size(); ++P)
@@ -685,6 +689,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
       pl.units.push_back(std::move(u));
     }
   CK(cudaStreamSynchronize(s));
+  pl.stats.plan_ms_units = lap();
   eri_stats_t& st = pl.stats;
   st.nshell = nshell; st.nao = b.nao; st.nao_cart = b.nao_cart; st.natm = natm;
   st.n_shell_groups = ng; st.n_pair_classes = (int)pl.pcs.size(); st.n_quartet_classes = (int)pl.units.size();

@@ -275,18 +275,219 @@ __global__ void __launch_bounds__(32 * WARPS, ((EM == 0 && WARPS == 4 && LD == 0
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// EM = 2, "team": the heaviest classes ((gg|fd) ... (gg|gg): more than 10 000 Cartesian elements; raised slab of all roots up
+// to 233 KB).  The block is ONE group of TW warps on one quartet: the elements are dealt over all 32 TW lanes (element
+// mode), and the roots are processed in chunks of RCH so that the slab of a chunk fits shared memory -- the roots of the
+// quadrature are independent terms of Eq. 1, so a chunk is built (phase 1), consumed (phase 2) and overwritten.
+// This replaces the generic thread-per-quartet kernel (86 KB of local memory per thread) for these classes.
+template <int LA, int LB, int LC, int LD, int TW>
+struct CoopGradTeamTraits {
+  static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+  static constexpr int NAB = NA * NB, NCD = NC * ND;
+  static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
+  static constexpr int SCD = ((LC + 2) * (LD + 1)) | 1, G2 = ((LA + 2) * (LB + 2) * SCD) | 1;
+  static constexpr int NDQ = NAB + NA * NC + NA * ND + NB * NC + NB * ND + NCD;   // the six density blocks of the quartet
+  static constexpr int BUDGET = 200 * 1024 / 8 - NDQ - 18 * TW;                    // doubles left for the slab
+  static constexpr int RCH = (BUDGET / (3 * G2) < N) ? BUDGET / (3 * G2) : N;       // roots per chunk
+  static_assert(RCH >= 1, "one root's slab does not fit");
+  static constexpr int SLAB2D = 3 * RCH * G2;
+  static constexpr int BASE = SLAB2D > TW * 32 * 33 ? SLAB2D : TW * 32 * 33;        // the dead slab stages the warp reductions
+  static constexpr int SLAB = BASE + NDQ + 18 * TW;
+  static constexpr size_t SMEM = sizeof(double) * SLAB;
+  static_assert(SMEM <= 227 * 1024, "slab does not fit");
+  static_assert(3 * RCH <= 32 * TW, "one lane per (root, axis) of a chunk");
+};
+
+template <int LA, int LB, int LC, int LD, int TW>
+__global__ void __launch_bounds__(32 * TW) coop_grad_team_kernel(Work w) {
+  using Tr = CoopGradTeamTraits<LA, LB, LC, LD, TW>;
+  constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, NAB = Tr::NAB, NCD = Tr::NCD;
+  constexpr int N = Tr::N, SCD = Tr::SCD, G2 = Tr::G2, RCH = Tr::RCH, T = 32 * TW;
+  constexpr int SK = LD + 1, SJ = SCD, SI = (LB + 2) * SCD;
+  extern __shared__ __align__(16) double smem[];
+  const int lane = threadIdx.x, wy = threadIdx.y, tid = wy * 32 + lane;
+  double* S = smem;
+  double* sDab = S + Tr::BASE; double* sDac = sDab + NAB; double* sDad = sDac + NA * NC; double* sDbc = sDad + NA * ND;
+  double* sDbd = sDbc + NB * NC; double* sDcd = sDbd + NB * ND; double* part = sDcd + NCD;
+
+  const PairSet& bp = w.bra; const PairSet& kp = w.ket;
+  const int blk = blockIdx.x * w.nshard + w.shard;
+  if (blk >= w.row_off[w.nrows]) return;
+  const int r = find_row_warp(w.row_off, w.nrows, blk, lane);
+  const int j = blk - w.row_off[r];                  // one ket pair per block
+  const int i_begin = r * w.grad_ch, i_end = min(i_begin + w.grad_ch, bp.npair);
+  if (j >= kp.npair) return;
+  const int n = w.nao;
+  const double* __restrict__ D = w.D;
+  double C[3], CD[3];
+#pragma unroll
+  for (int x = 0; x < 3; ++x) { C[x] = kp.geom[x * kp.stride + j]; CD[x] = kp.geom[(3 + x) * kp.stride + j]; }
+  const double wket = kp.geom[6 * kp.stride + j];
+  const int c0 = kp.ao[j].x, d0 = kp.ao[j].y;
+  for (int cd = tid; cd < NCD; cd += T) sDcd[cd] = D[(long)(c0 + cd / ND) * n + d0 + cd % ND];
+  double keepC = 0.0, keepD = 0.0;   // warp 0, lane v < 18
+
+  for (int i = i_begin; i < i_end; ++i) {
+    if (j >= w.ket_count[i]) continue;     // block-uniform
+    double f = bp.geom[6 * bp.stride + i] * wket;
+    if (w.same && i == j) f *= 0.5;
+    double A[3], AB[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) { A[x] = bp.geom[x * bp.stride + i]; AB[x] = bp.geom[(3 + x) * bp.stride + i]; }
+    const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
+    __syncthreads();
+    for (int e = tid; e < NAB; e += T) sDab[e] = D[(long)(a0 + e / NB) * n + b0 + e % NB];
+    for (int e = tid; e < NA * NC; e += T) sDac[e] = D[(long)(a0 + e / NC) * n + c0 + e % NC];
+    for (int e = tid; e < NA * ND; e += T) sDad[e] = D[(long)(a0 + e / ND) * n + d0 + e % ND];
+    for (int e = tid; e < NB * NC; e += T) sDbc[e] = D[(long)(b0 + e / NC) * n + c0 + e % NC];
+    for (int e = tid; e < NB * ND; e += T) sDbd[e] = D[(long)(b0 + e / ND) * n + d0 + e % ND];
+
+    double acc[18];
+#pragma unroll
+    for (int e = 0; e < 18; ++e) acc[e] = 0.0;
+
+    for (int kb = 0; kb < bp.npp; ++kb) {
+      const double p = bp.prim[(kb * 5 + 0) * bp.stride + i];
+      const double P[3] = {bp.prim[(kb * 5 + 1) * bp.stride + i], bp.prim[(kb * 5 + 2) * bp.stride + i], bp.prim[(kb * 5 + 3) * bp.stride + i]};
+      const double Kab = bp.prim[(kb * 5 + 4) * bp.stride + i];
+      const double ea2 = 2.0 * bp.aexp[(kb * 2 + 0) * bp.stride + i], eb2 = 2.0 * bp.aexp[(kb * 2 + 1) * bp.stride + i];
+      bool swb;
+      {
+        double da = 0.0, db = 0.0;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { const double pa = P[x] - A[x], pb = pa + AB[x]; da += pa * pa; db += pb * pb; }
+        swb = db < da;
+      }
+      for (int kk = 0; kk < kp.npp; ++kk) {
+        const double q = kp.prim[(kk * 5 + 0) * kp.stride + j];
+        const double Q[3] = {kp.prim[(kk * 5 + 1) * kp.stride + j], kp.prim[(kk * 5 + 2) * kp.stride + j], kp.prim[(kk * 5 + 3) * kp.stride + j]};
+        const double Kcd = kp.prim[(kk * 5 + 4) * kp.stride + j];
+        const double ec2 = 2.0 * kp.aexp[(kk * 2 + 0) * kp.stride + j];
+        bool swk = false;
+        if (LD > 0) {
+          double dc = 0.0, dd = 0.0;
+#pragma unroll
+          for (int x = 0; x < 3; ++x) { const double qc = Q[x] - C[x], qd = qc + CD[x]; dc += qc * qc; dd += qd * qd; }
+          swk = dd < dc;
+        }
+        const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+        const double PQ[3] = {P[0] - Q[0], P[1] - Q[1], P[2] - Q[2]};
+        const double xx = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
+#pragma unroll 1
+        for (int r0 = 0; r0 < N; r0 += RCH) {
+          const int nr = min(RCH, N - r0);
+          // ---- phase 1: lane (root of the chunk, axis) ----
+          __syncthreads();
+          if (tid < 3 * nr) {
+            const int rl = tid / 3, ax = tid - 3 * rl;
+            double u, wt;
+            rys_root_one<N>(xx, w.rys, r0 + rl, u, wt);
+            const double t2 = u * rpq;
+            const double b00 = 0.5 * t2, b10 = (1.0 - q * t2) * 0.5 / p, b01 = (1.0 - p * t2) * 0.5 / q;
+            const double pa = (ax == 0 ? P[0] - A[0] : ax == 1 ? P[1] - A[1] : P[2] - A[2]);
+            const double qc = (ax == 0 ? Q[0] - C[0] : ax == 1 ? Q[1] - C[1] : Q[2] - C[2]);
+            const double pqx = (ax == 0 ? PQ[0] : ax == 1 ? PQ[1] : PQ[2]);
+            const double abx = (ax == 0 ? AB[0] : ax == 1 ? AB[1] : AB[2]);
+            const double cdx = (ax == 0 ? CD[0] : ax == 1 ? CD[1] : CD[2]);
+            const double c00 = pa + (swb ? abx : 0.0) - q * t2 * pqx;
+            const double c00p = qc + (swk ? cdx : 0.0) + p * t2 * pqx;
+            const double init = ax == 2 ? f * Kab * Kcd * sqrt(rpq) * wt : 1.0;
+            double* dst = S + (ax * RCH + rl) * G2;
+            if (!swb) {
+              if (!swk) fill_2d_smem<LA + 1, LB + 1, LC + 1, LD>(dst, SI, SJ, SK, 1, init, c00, c00p, b10, b01, b00, abx, cdx);
+              else if constexpr (LD > 0) fill_2d_smem<LA + 1, LB + 1, LD, LC + 1>(dst, SI, SJ, 1, SK, init, c00, c00p, b10, b01, b00, abx, -cdx);
+            } else {
+              if (!swk) fill_2d_smem<LB + 1, LA + 1, LC + 1, LD>(dst, SJ, SI, SK, 1, init, c00, c00p, b10, b01, b00, -abx, cdx);
+              else if constexpr (LD > 0) fill_2d_smem<LB + 1, LA + 1, LD, LC + 1>(dst, SJ, SI, 1, SK, init, c00, c00p, b10, b01, b00, -abx, -cdx);
+            }
+          }
+          __syncthreads();
+          // ---- phase 2: the Cartesian elements dealt over all lanes of the block ----
+#pragma unroll 1
+          for (int e = tid; e < NAB * NCD; e += T) {
+            const int id = e % ND, t1 = e / ND, ic = t1 % NC, t2 = t1 / NC, ib = t2 % NB, ia = t2 / NB;
+            int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
+            cart_powers(LA, ia, ax, ay, az); cart_powers(LB, ib, bx, by, bz); cart_powers(LC, ic, cx, cy, cz); cart_powers(LD, id, dx, dy, dz);
+            const double pj = sDab[ia * NB + ib] * sDcd[ic * ND + id];
+            const double pk = fma(sDac[ia * NC + ic], sDbd[ib * ND + id], sDad[ia * ND + id] * sDbc[ib * NC + ic]);
+            const int ox = ax * SI + bx * SJ + cx * SK + dx, oy = ay * SI + by * SJ + cy * SK + dy + RCH * G2, oz = az * SI + bz * SJ + cz * SK + dz + 2 * RCH * G2;
+            const int lax = ax > 0 ? -SI : 0, lay = ay > 0 ? -SI : 0, laz = az > 0 ? -SI : 0;
+            const int lbx = bx > 0 ? -SJ : 0, lby = by > 0 ? -SJ : 0, lbz = bz > 0 ? -SJ : 0;
+            const int lcx = cx > 0 ? -SK : 0, lcy = cy > 0 ? -SK : 0, lcz = cz > 0 ? -SK : 0;
+            const double fax = ax, fay = ay, faz = az, fbx = bx, fby = by, fbz = bz, fcx = cx, fcy = cy, fcz = cz;
+#pragma unroll 1
+            for (int rt = 0; rt < nr; ++rt) {
+              const double* X = S + ox + rt * G2;
+              const double* Y = S + oy + rt * G2;
+              const double* Z = S + oz + rt * G2;
+              const double vx = X[0], vy = Y[0], vz = Z[0];
+              const double oyz = vy * vz, oxz = vx * vz, oxy = vx * vy;
+              const double dAx = fma(ea2, X[SI], -fax * X[lax]), dAy = fma(ea2, Y[SI], -fay * Y[lay]), dAz = fma(ea2, Z[SI], -faz * Z[laz]);
+              const double dBx = fma(eb2, X[SJ], -fbx * X[lbx]), dBy = fma(eb2, Y[SJ], -fby * Y[lby]), dBz = fma(eb2, Z[SJ], -fbz * Z[lbz]);
+              const double dCx = fma(ec2, X[SK], -fcx * X[lcx]), dCy = fma(ec2, Y[SK], -fcy * Y[lcy]), dCz = fma(ec2, Z[SK], -fcz * Z[lcz]);
+              const double jx = pj * oyz, jy = pj * oxz, jz = pj * oxy;
+              const double kx = pk * oyz, ky = pk * oxz, kz = pk * oxy;
+              acc[0] = fma(dAx, jx, acc[0]); acc[1] = fma(dAy, jy, acc[1]); acc[2] = fma(dAz, jz, acc[2]);
+              acc[3] = fma(dBx, jx, acc[3]); acc[4] = fma(dBy, jy, acc[4]); acc[5] = fma(dBz, jz, acc[5]);
+              acc[6] = fma(dCx, jx, acc[6]); acc[7] = fma(dCy, jy, acc[7]); acc[8] = fma(dCz, jz, acc[8]);
+              acc[9] = fma(dAx, kx, acc[9]); acc[10] = fma(dAy, ky, acc[10]); acc[11] = fma(dAz, kz, acc[11]);
+              acc[12] = fma(dBx, kx, acc[12]); acc[13] = fma(dBy, ky, acc[13]); acc[14] = fma(dBz, kz, acc[14]);
+              acc[15] = fma(dCx, kx, acc[15]); acc[16] = fma(dCy, ky, acc[16]); acc[17] = fma(dCz, kz, acc[17]);
+            }
+          }
+        }
+      }
+    }
+    // ---- phase 3: sum over the lanes of each warp through the dead slab, then over the warps ----
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { acc[e] *= 4.0; acc[9 + e] *= 2.0; }
+    __syncthreads();
+    if (lane < 18) part[wy * 18 + lane] = 0.0;
+    warp_reduce_values<18, false>(acc, S + wy * (32 * 33), lane, [&](int v, int, double sum) { part[wy * 18 + v] = sum; });
+    __syncthreads();
+    if (wy == 0 && lane < 18) {
+      double sum = 0.0;
+#pragma unroll
+      for (int ww = 0; ww < TW; ++ww) sum += part[ww * 18 + lane];
+      const int2 at_ab = bp.atom[i];
+      const int jk = lane / 9, ce = (lane % 9) / 3, ax = lane % 3;
+      if (ce < 2) atomic_add((jk ? w.gK : w.gJ) + 3 * (ce == 0 ? at_ab.x : at_ab.y) + ax, sum);
+      else keepC += sum;
+      keepD -= sum;
+    }
+  }
+  if (wy == 0 && lane < 18) {
+    const int jk = lane / 9, ax = lane % 3;
+    const int2 at_cd = kp.atom[j];
+    double* gout = jk ? w.gK : w.gJ;
+    if (keepC != 0.0) atomic_add(gout + 3 * at_cd.x + ax, keepC);
+    if (keepD != 0.0) atomic_add(gout + 3 * at_cd.y + ax, keepD);
+  }
+}
+
 template <int LA, int LB, int LC, int LD, int WARPS, int EM>
 cudaError_t launch_coop_grad(const Work& w, int nblocks_dense, cudaStream_t s) {
-  using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS, EM>;
   const int grid = (nblocks_dense + w.nshard - 1) / w.nshard;
   if (grid <= 0) return cudaSuccess;
   static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(coop_grad_kernel<LA, LB, LC, LD, WARPS, EM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
+  if constexpr (EM == 2) {
+    using Tr = CoopGradTeamTraits<LA, LB, LC, LD, WARPS>;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(coop_grad_team_kernel<LA, LB, LC, LD, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    coop_grad_team_kernel<LA, LB, LC, LD, WARPS><<<grid, dim3(32, WARPS), Tr::SMEM, s>>>(w);
+  } else {
+    using Tr = CoopGradTraits<LA, LB, LC, LD, WARPS, EM>;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(coop_grad_kernel<LA, LB, LC, LD, WARPS, EM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    coop_grad_kernel<LA, LB, LC, LD, WARPS, EM><<<grid, dim3(32, WARPS), Tr::SMEM, s>>>(w);
   }
-  coop_grad_kernel<LA, LB, LC, LD, WARPS, EM><<<grid, dim3(32, WARPS), Tr::SMEM, s>>>(w);
   return cudaGetLastError();
 }
 

@@ -14,7 +14,7 @@
 
 namespace eri {
 
-template <int LA, int LB, int LC, int LD, int BI>
+template <int LA, int LB, int LC, int LD, int BI, int MODE = 0>
 struct TileGradTraits {
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
   static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
@@ -22,7 +22,8 @@ struct TileGradTraits {
   static constexpr int NUNI = NA * NB + 2 * (NA * NC + NB * NC);                 // D_ab per warp; D_ac, D_bc per ket half
   static constexpr int NLANE = NC * ND + NA * ND + NB * ND;                       // D_cd, D_ad, D_bd: per lane
   static constexpr int STAGE = 32 * 33;
-  static constexpr int PERWARP = STAGE + NUNI + 32 * NLANE;
+  static constexpr int NE = NA * NB * NC * ND;
+  static constexpr int PERWARP = STAGE + NUNI + 32 * NLANE + (MODE == 3 ? 2 * NE * 32 : 0);   // MODE 3: + the pj, pk columns
   static constexpr int RT = rys2_size(N);                    // the class's Rys table, first in the block's shared memory
   static constexpr size_t SMEM = sizeof(double) * (RT + BI * PERWARP);
 };
@@ -91,9 +92,60 @@ __device__ __forceinline__ void tile_grad_axis(double* __restrict__ acc, const d
   }
 }
 
+// one differentiated axis of one root with the density products pj[e], pk[e] of the quartet read from a shared-memory column
+// (pjk[32 e], pjk[32 (NE + e)]); accumulates [J: A, B, C | K: A, B, C] of axis AX (MODE 2 and MODE 3)
+template <int LA, int LB, int LC, int LD, int AX>
+__device__ __forceinline__ void tile_grad_team_axis(double* __restrict__ acc, const double* c00, const double* c00p, const double* init,
+                                                    double b10, double b01, double b00, const double* AB, const double* CD,
+                                                    double ea2, double eb2, double ec2, const double* __restrict__ pjk) {
+  constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD), NE = NA * NB * NC * ND;
+  constexpr int G2R = (LA + 2) * (LB + 2) * (LC + 2) * (LD + 1), G2B = (LA + 1) * (LB + 1) * (LC + 1) * (LD + 1);
+  constexpr int RC = LD + 1, RB = (LC + 2) * RC, RA = (LB + 2) * RB;     // raised strides
+  constexpr int PC = LD + 1, PB = (LC + 1) * PC, PA = (LB + 1) * PB;     // plain strides
+  constexpr int O1 = (AX + 1) % 3, O2 = (AX + 2) % 3;
+  double gr[G2R], g1[G2B], g2[G2B];
+  fill_2d_tile<LA + 1, LB + 1, LC + 1, LD>(gr, init[AX], c00[AX], c00p[AX], b10, b01, b00, AB[AX], CD[AX]);
+  fill_2d_tile<LA, LB, LC, LD>(g1, init[O1], c00[O1], c00p[O1], b10, b01, b00, AB[O1], CD[O1]);
+  fill_2d_tile<LA, LB, LC, LD>(g2, init[O2], c00[O2], c00p[O2], b10, b01, b00, AB[O2], CD[O2]);
+  int e = 0;
+#pragma unroll
+  for (int ax = LA; ax >= 0; --ax)
+#pragma unroll
+  for (int ay = LA - ax; ay >= 0; --ay) {
+    const int pa[3] = {ax, ay, LA - ax - ay};
+#pragma unroll
+    for (int bx = LB; bx >= 0; --bx)
+#pragma unroll
+    for (int by = LB - bx; by >= 0; --by) {
+      const int pb[3] = {bx, by, LB - bx - by};
+#pragma unroll
+      for (int cx = LC; cx >= 0; --cx)
+#pragma unroll
+      for (int cy = LC - cx; cy >= 0; --cy) {
+        const int pc[3] = {cx, cy, LC - cx - cy};
+#pragma unroll
+        for (int dx = LD; dx >= 0; --dx)
+#pragma unroll
+        for (int dy = LD - dx; dy >= 0; --dy) {
+          const int pd[3] = {dx, dy, LD - dx - dy};
+          const int er = pa[AX] * RA + pb[AX] * RB + pc[AX] * RC + pd[AX];
+          const double oth = g1[pa[O1] * PA + pb[O1] * PB + pc[O1] * PC + pd[O1]] * g2[pa[O2] * PA + pb[O2] * PB + pc[O2] * PC + pd[O2]];
+          const double dA = pa[AX] > 0 ? fma(ea2, gr[er + RA], -pa[AX] * gr[er - RA]) : ea2 * gr[er + RA];
+          const double dB = pb[AX] > 0 ? fma(eb2, gr[er + RB], -pb[AX] * gr[er - RB]) : eb2 * gr[er + RB];
+          const double dC = pc[AX] > 0 ? fma(ec2, gr[er + RC], -pc[AX] * gr[er - RC]) : ec2 * gr[er + RC];
+          const double tj = pjk[32 * e] * oth, tk = pjk[32 * (NE + e)] * oth;
+          acc[0] = fma(dA, tj, acc[0]); acc[1] = fma(dB, tj, acc[1]); acc[2] = fma(dC, tj, acc[2]);
+          acc[3] = fma(dA, tk, acc[3]); acc[4] = fma(dB, tk, acc[4]); acc[5] = fma(dC, tk, acc[5]);
+          ++e;
+        }
+      }
+    }
+  }
+}
+
 template <int LA, int LB, int LC, int LD, int BI, int MODE>
 __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
-  using Tr = TileGradTraits<LA, LB, LC, LD, BI>;
+  using Tr = TileGradTraits<LA, LB, LC, LD, BI, MODE>;
   constexpr int NA = Tr::NA, NB = Tr::NB, NC = Tr::NC, ND = Tr::ND, N = Tr::N, G2 = Tr::G2;
   constexpr int SD = 1, SC = LD + 1, SB = (LC + 2) * SC, SA = (LB + 2) * SB;   // strides of the raised 2-D arrays
   extern __shared__ __align__(16) double smem[];
@@ -156,6 +208,17 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
 #pragma unroll
       for (int d = 0; d < ND; ++d) Dbd_s[32 * (b * ND + d)] = D[(long)(b0 + b) * n + d0 + d];
     __syncwarp();
+    [[maybe_unused]] double* pjk = mine + 32 * Tr::NLANE;   // MODE 3: pj[e] at 32 e, pk[e] at 32 (NE + e), column of this lane
+    if constexpr (MODE == 3) {
+      // the density products of the row's quartets once, in shared memory: held in registers across the three axis passes they
+      // spilled (profiles/r02_cfg4.md); run-time element index, the loop is short and not unrolled
+#pragma unroll 1
+      for (int e = 0; e < Tr::NE; ++e) {
+        const int d = e % ND, t1 = e / ND, c = t1 % NC, t2 = t1 / NC, b = t2 % NB, a = t2 / NB;
+        pjk[32 * e] = Dab_s[a * NB + b] * Dcd_s[32 * (c * ND + d)];
+        pjk[32 * (Tr::NE + e)] = fma(Dac_s[a * NC + c], Dbd_s[32 * (b * ND + d)], Dad_s[32 * (a * ND + d)] * Dbc_s[b * NC + c]);
+      }
+    }
 
     double acc[18];   // [J: A xyz, B xyz, C xyz | K: same]
 #pragma unroll
@@ -187,7 +250,27 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
           const double hq = 0.5 / q;
           double u[N], wt[N];
           rys_roots_smem<N>(xx, rtab, w.rys, u, wt);
-          if constexpr (MODE == 1) {
+          if constexpr (MODE == 3) {
+#pragma unroll 1
+            for (int rt = 0; rt < N; ++rt) {
+              const double t2 = u[rt] * rpq;
+              const double b00 = 0.5 * t2, b10 = hp - q * t2 * hp, b01 = hq - p * t2 * hq;
+              const double c00[3] = {(P[0] - A[0]) - q * t2 * PQ[0], (P[1] - A[1]) - q * t2 * PQ[1], (P[2] - A[2]) - q * t2 * PQ[2]};
+              const double c00p[3] = {(Q[0] - C[0]) + p * t2 * PQ[0], (Q[1] - C[1]) + p * t2 * PQ[1], (Q[2] - C[2]) + p * t2 * PQ[2]};
+              const double init[3] = {1.0, 1.0, pref * wt[rt]};
+              double a6[6];
+#pragma unroll
+              for (int ax = 0; ax < 3; ++ax) {
+#pragma unroll
+                for (int e = 0; e < 6; ++e) a6[e] = 0.0;
+                if (ax == 0) tile_grad_team_axis<LA, LB, LC, LD, 0>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
+                else if (ax == 1) tile_grad_team_axis<LA, LB, LC, LD, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
+                else tile_grad_team_axis<LA, LB, LC, LD, 2>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
+#pragma unroll
+                for (int e = 0; e < 6; ++e) acc[(e / 3) * 9 + (e % 3) * 3 + ax] += a6[e];
+              }
+            }
+          } else if constexpr (MODE == 1) {
 #pragma unroll 1
             for (int rt = 0; rt < N; ++rt) {
               const double t2 = u[rt] * rpq;
@@ -319,55 +402,6 @@ struct TileGradTeamTraits {
   static constexpr int RT = rys2_size(N);
   static constexpr size_t SMEM = sizeof(double) * (RT + BI * PERTEAM);
 };
-
-template <int LA, int LB, int LC, int LD, int AX>
-__device__ __forceinline__ void tile_grad_team_axis(double* __restrict__ acc, const double* c00, const double* c00p, const double* init,
-                                                    double b10, double b01, double b00, const double* AB, const double* CD,
-                                                    double ea2, double eb2, double ec2, const double* __restrict__ pjk) {
-  constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD), NE = NA * NB * NC * ND;
-  constexpr int G2R = (LA + 2) * (LB + 2) * (LC + 2) * (LD + 1), G2B = (LA + 1) * (LB + 1) * (LC + 1) * (LD + 1);
-  constexpr int RC = LD + 1, RB = (LC + 2) * RC, RA = (LB + 2) * RB;     // raised strides
-  constexpr int PC = LD + 1, PB = (LC + 1) * PC, PA = (LB + 1) * PB;     // plain strides
-  constexpr int O1 = (AX + 1) % 3, O2 = (AX + 2) % 3;
-  double gr[G2R], g1[G2B], g2[G2B];
-  fill_2d_tile<LA + 1, LB + 1, LC + 1, LD>(gr, init[AX], c00[AX], c00p[AX], b10, b01, b00, AB[AX], CD[AX]);
-  fill_2d_tile<LA, LB, LC, LD>(g1, init[O1], c00[O1], c00p[O1], b10, b01, b00, AB[O1], CD[O1]);
-  fill_2d_tile<LA, LB, LC, LD>(g2, init[O2], c00[O2], c00p[O2], b10, b01, b00, AB[O2], CD[O2]);
-  int e = 0;
-#pragma unroll
-  for (int ax = LA; ax >= 0; --ax)
-#pragma unroll
-  for (int ay = LA - ax; ay >= 0; --ay) {
-    const int pa[3] = {ax, ay, LA - ax - ay};
-#pragma unroll
-    for (int bx = LB; bx >= 0; --bx)
-#pragma unroll
-    for (int by = LB - bx; by >= 0; --by) {
-      const int pb[3] = {bx, by, LB - bx - by};
-#pragma unroll
-      for (int cx = LC; cx >= 0; --cx)
-#pragma unroll
-      for (int cy = LC - cx; cy >= 0; --cy) {
-        const int pc[3] = {cx, cy, LC - cx - cy};
-#pragma unroll
-        for (int dx = LD; dx >= 0; --dx)
-#pragma unroll
-        for (int dy = LD - dx; dy >= 0; --dy) {
-          const int pd[3] = {dx, dy, LD - dx - dy};
-          const int er = pa[AX] * RA + pb[AX] * RB + pc[AX] * RC + pd[AX];
-          const double oth = g1[pa[O1] * PA + pb[O1] * PB + pc[O1] * PC + pd[O1]] * g2[pa[O2] * PA + pb[O2] * PB + pc[O2] * PC + pd[O2]];
-          const double dA = pa[AX] > 0 ? fma(ea2, gr[er + RA], -pa[AX] * gr[er - RA]) : ea2 * gr[er + RA];
-          const double dB = pb[AX] > 0 ? fma(eb2, gr[er + RB], -pb[AX] * gr[er - RB]) : eb2 * gr[er + RB];
-          const double dC = pc[AX] > 0 ? fma(ec2, gr[er + RC], -pc[AX] * gr[er - RC]) : ec2 * gr[er + RC];
-          const double tj = pjk[32 * e] * oth, tk = pjk[32 * (NE + e)] * oth;
-          acc[0] = fma(dA, tj, acc[0]); acc[1] = fma(dB, tj, acc[1]); acc[2] = fma(dC, tj, acc[2]);
-          acc[3] = fma(dA, tk, acc[3]); acc[4] = fma(dB, tk, acc[4]); acc[5] = fma(dC, tk, acc[5]);
-          ++e;
-        }
-      }
-    }
-  }
-}
 
 template <int LA, int LB, int LC, int LD, int BI>
 __global__ void __launch_bounds__(96 * BI) tile_grad_team_kernel(Work w) {
@@ -528,7 +562,8 @@ cudaError_t launch_tile_grad(const Work& w, int nblocks_dense, cudaStream_t s) {
     }
     tile_grad_team_kernel<LA, LB, LC, LD, BI><<<grid, dim3(32, 3 * BI), Tr::SMEM, s>>>(w);
   } else {
-    using Tr = TileGradTraits<LA, LB, LC, LD, BI>;
+    using Tr = TileGradTraits<LA, LB, LC, LD, BI, MODE>;
+    static_assert(Tr::SMEM <= 227 * 1024, "tile gradient kernel: shared memory");
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(tile_grad_kernel<LA, LB, LC, LD, BI, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM);
       if (e != cudaSuccess) return e;

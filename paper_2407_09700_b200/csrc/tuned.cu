@@ -103,7 +103,7 @@ static_assert(CGRAD_NGROUPS == 8, "tuned.cu lists eight cooperative gradient gro
 // cooperative gradient kernel (kind 2): Schwarz-sorted pair sets, task = 16 bra pairs x 1 ket pair, `warps` ket pairs per block
 bool coop_grad_info(int la, int lb, int lc, int ld, TunedInfo* info) {
   switch (la * 1000 + lb * 100 + lc * 10 + ld) {
-#define X(a, b, c, d, wp, em) case a * 1000 + b * 100 + c * 10 + d: info->kind = 2; info->TQ = 1; info->BI = 16; info->BJ = wp; return true;
+#define X(a, b, c, d, wp, em) case a * 1000 + b * 100 + c * 10 + d: info->kind = 2; info->TQ = 1; info->BI = 16; info->BJ = (em == 2 ? 1 : wp); return true;   // EM = 2: the block is one team on one ket pair
     CGRAD_ALL(X)
 #undef X
     default: return false;

@@ -27,7 +27,8 @@ class eri_stats_t(ctypes.Structure):
     _fields_ = [("nshell", _i32), ("nao", _i32), ("nao_cart", _i32), ("natm", _i32), ("n_shell_groups", _i32),
                 ("n_pair_classes", _i32), ("n_quartet_classes", _i32), ("launches_per_call", _i32),
                 ("pairs_total", _i64), ("pairs_kept", _i64), ("quartets_total", _i64), ("quartets_kept", _i64),
-                ("canonical_flops", _f64), ("canonical_flops_grad", _f64), ("plan_ms", _f64)]
+                ("canonical_flops", _f64), ("canonical_flops_grad", _f64), ("plan_ms", _f64),
+                ("plan_ms_init", _f64), ("plan_ms_schwarz", _f64), ("plan_ms_pairs", _f64), ("plan_ms_units", _f64)]
 
 
 class eri_class_stat_t(ctypes.Structure):
