@@ -1,7 +1,7 @@
 /* eri.h -- C ABI of liberi_b200.so: integral-direct J/K build and J/K nuclear gradient on one B200 (sm_100a).
  *
  * What is computed (citations are lines of the paper text, PAPER.md, of arxiv 2407.09700):
- *   contracted four-centre electron-repulsion integrals over Gaussian shells with l <= 4 by Rys quadrature
+ *   contracted four-centre electron-repulsion integrals over Gaussian shells with l <= 6 by Rys quadrature
  *   (Eq. 1-5), digested on the fly with a density matrix into the Coulomb and exchange matrices
  *   by the six updates of Algorithm 2 lines 8-13, read as full sums:
  *       J_ij = sum_kl (ij|kl) D_kl,     K_ik = sum_jl (ij|kl) D_jl,
@@ -28,8 +28,8 @@
  * Devices: the library binds to the CUDA device that is current at its first compute call (its Rys tables, the
  * constant-memory transform table and the kernels' shared-memory attributes live there).  Calling any compute entry point
  * while another device is current returns ERI_ERR_BAD_ARG; one process drives one GPU (multi-GPU: one process per GPU,
- * eri_plan_set_shard).  eri_plan_set_kernel_mode re-uploads the plan's row tables and blocks the host until that is done
- * (on a private stream: no device-wide synchronisation).
+ * eri_plan_set_shard).  eri_plan_set_kernel_mode and eri_plan_set_tuning wait for the device, re-upload the plan's row
+ * tables and block the host until that is done (rare calls, like plan creation).
  *
  * Errors: every int-returning function returns ERI_OK (0) or a negative code and never throws; the message of the
  * last failure in the calling thread is available through eri_last_error().  There is no CPU fallback: without a
@@ -46,10 +46,10 @@ extern "C" {
 
 #define ERI_OK 0
 #define ERI_ERR_BAD_ARG (-1)       /* null pointer, nprim <= 0, exponent <= 0, inconsistent ao_off / prim_off / atom */
-#define ERI_ERR_UNSUPPORTED_L (-2) /* l < 0 or l > 4 */
+#define ERI_ERR_UNSUPPORTED_L (-2) /* l < 0 or l > ERI_LMAX */
 #define ERI_ERR_CUDA (-3)          /* any CUDA runtime failure, including "no device" */
 #define ERI_ERR_NOMEM (-4)         /* host or device allocation failed */
-#define ERI_LMAX 4
+#define ERI_LMAX 6   /* s, p, d, f, g with tuned kernels; h and i (the paper stops at g) on the generic kernels */
 
 typedef struct { int32_t atom; int32_t l; int32_t nprim; int32_t prim_off; int32_t ao_off; } eri_shell_t;
 typedef struct { double exp; double coef; } eri_prim_t;
@@ -144,7 +144,7 @@ int eri_plan_set_tuning(eri_plan_t* plan, int key, double value);
  * class launch (quartets are independent units).  The outputs are then PARTIAL sums; J, K and the gradient
  * are linear in them, so the caller sums the outputs over ranks (one all-reduce).  Default rank 0 of 1. */
 int eri_plan_set_shard(eri_plan_t* plan, int rank, int nranks);
-void eri_plan_destroy(eri_plan_t* plan);
+void eri_plan_destroy(eri_plan_t* plan);   /* waits for the device to finish, then releases the plan's buffers */
 
 /* ---- diagnostics / benchmark entry points -------------------------------------------------------------------- */
 /* Spherical ERI blocks (ij|kl) for an explicit list of shell quartets (any order of shells).  Block n is written

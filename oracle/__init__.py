@@ -45,7 +45,7 @@ def lib():
         _lib.oracle_prim_eri.restype = ctypes.c_double
         _lib.oracle_jk.restype = ctypes.c_longlong
         _lib.oracle_jk_dscreen.restype = ctypes.c_longlong
-        for l in range(5):
+        for l in range(7):
             T = sph.c2s(l)
             _lib.oracle_set_c2s(l, _d(T))
     return _lib

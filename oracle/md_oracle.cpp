@@ -37,8 +37,8 @@
 
 namespace {
 
-constexpr int LMAX = 4;          // g
-constexpr int LTOT_MAX = 4 * LMAX + 1;  // 17 with one raised index (gradient)
+constexpr int LMAX = 6;          // i (capacity only: array bounds, no arithmetic depends on it)
+constexpr int LTOT_MAX = 4 * LMAX + 1;  // 25 with one raised index (gradient)
 
 struct Shell { int32_t atom, l, nprim, prim_off, ao_off; };
 struct Prim { double e, c; };

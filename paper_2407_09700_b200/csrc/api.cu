@@ -39,6 +39,28 @@ int fail(int code, const char* fmt, ...) {
   } while (0)
 #define CKI(call) do { int r_ = (call); if (r_ != ERI_OK) return r_; } while (0)
 
+// Device allocations go through the stream-ordered allocator on a private stream with the pool's release threshold lifted:
+// a plan makes some thousand small allocations (pair sets, row tables), and cudaMalloc / cudaFree (each an implicit device
+// synchronisation) were a third of plan creation (profiles/r02_plan.md).  alloc() waits for its own allocation, so the
+// pointer is usable on any stream; release() is ordered on the private stream only, so every owner synchronises the streams
+// that used the buffer before it lets go of it (plan creation does; eri_plan_destroy synchronises the device first).
+cudaStream_t g_alloc_stream = nullptr;
+cudaError_t alloc_stream(cudaStream_t* out) {
+  static std::mutex mu;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!g_alloc_stream) {
+    cudaError_t e = cudaStreamCreateWithFlags(&g_alloc_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return e;
+    int dev = 0; cudaMemPool_t pool = nullptr;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      unsigned long long keep = ~0ull;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+  }
+  *out = g_alloc_stream;
+  return cudaSuccess;
+}
+
 template <class T>
 struct Dev {   // owning device array
   T* p = nullptr; size_t n = 0;
@@ -47,12 +69,17 @@ struct Dev {   // owning device array
   Dev(Dev&& o) noexcept : p(o.p), n(o.n) { o.p = nullptr; o.n = 0; }
   Dev& operator=(Dev&& o) noexcept { if (this != &o) { release(); p = o.p; n = o.n; o.p = nullptr; o.n = 0; } return *this; }
   ~Dev() { release(); }
-  void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+  void release() { if (p) { if (g_alloc_stream) cudaFreeAsync(p, g_alloc_stream); else cudaFree(p); } p = nullptr; n = 0; }
   cudaError_t alloc(size_t count) {
     release();
     if (count == 0) return cudaSuccess;
+    cudaStream_t as = nullptr;
+    cudaError_t e = alloc_stream(&as);
+    if (e != cudaSuccess) return e;
+    e = cudaMallocAsync(&p, count * sizeof(T), as);
+    if (e != cudaSuccess) { p = nullptr; return e; }
     n = count;
-    return cudaMalloc(&p, count * sizeof(T));
+    return cudaStreamSynchronize(as);
   }
   cudaError_t upload(const std::vector<T>& h, cudaStream_t s) {
     cudaError_t e = alloc(h.size());
@@ -109,6 +136,7 @@ int ensure_init() {
     return fail(ERI_ERR_BAD_ARG, "liberi_b200 is bound to CUDA device %d (current at its first call) but device %d is current", g_device, dev);
   if (!g_rys) {
     // consistency of the compile-time constants in eri_dev.cuh with the generated table
+    static_assert(RYS_NMAX == RYS_NROOTS_MAX, "rys_tables.inc must tabulate N = 1..RYS_NROOTS_MAX");
     for (int N = 1; N <= RYS_NMAX; ++N)
       if (rys_offset(N) != RYS_TABLE_OFFSET_H[N] || rys_xmax(N) != RYS_XMAX_H[N])
         return fail(ERI_ERR_BAD_ARG, "rys_tables.inc does not match eri_dev.cuh (N=%d)", N);
@@ -133,7 +161,8 @@ int ensure_init() {
   if (!g_c2s_ready) {
     std::vector<double> all;
     for (int l = 0; l <= LMAX; ++l) { build_c2s(l, g_c2s_host[l]); all.insert(all.end(), g_c2s_host[l].begin(), g_c2s_host[l].end()); }
-    if (all.size() != 245) return fail(ERI_ERR_BAD_ARG, "internal: c2s table size");
+    size_t want = 0; for (int l = 0; l <= LMAX; ++l) want += (size_t)nsph(l) * ncart(l);
+    if (all.size() != want) return fail(ERI_ERR_BAD_ARG, "internal: c2s table size");
     CK(upload_c2s(all.data()));
     g_c2s_ready = true;
   }
@@ -844,7 +873,7 @@ const char* eri_strerror(int code) {
   switch (code) {
     case ERI_OK: return "ok";
     case ERI_ERR_BAD_ARG: return "bad argument";
-    case ERI_ERR_UNSUPPORTED_L: return "angular momentum outside 0..4";
+    case ERI_ERR_UNSUPPORTED_L: return "angular momentum outside 0..6";
     case ERI_ERR_CUDA: return "CUDA failure";
     case ERI_ERR_NOMEM: return "out of memory";
     default: return "unknown error code";
@@ -881,7 +910,11 @@ int eri_list_plan_create(const eri_shell_t* shells, int nshell, const eri_prim_t
     catch (...) { return fail(ERI_ERR_BAD_ARG, "unexpected exception"); }
 }
 
-void eri_plan_destroy(eri_plan_t* plan) { delete plan; }
+void eri_plan_destroy(eri_plan_t* plan) {
+  if (!plan) return;
+  cudaDeviceSynchronize();   // the plan's buffers go back to the allocator's pool: nothing may still be using them
+  delete plan;
+}
 int eri_plan_set_shard(eri_plan_t* plan, int rank, int nranks) {
   if (!plan || nranks < 1 || rank < 0 || rank >= nranks) return fail(ERI_ERR_BAD_ARG, "bad shard %d of %d", rank, nranks);
   plan->shard = rank; plan->nshard = nranks;
@@ -986,8 +1019,9 @@ int eri_plan_class_stats(const eri_plan_t* cplan, eri_class_stat_t* out, int max
 }
 int eri_plan_set_timing(eri_plan_t* plan, int on) { if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan"); plan->timing = on; return ERI_OK; }
 static int reselect_kernels(eri_plan_t* plan) {
-  // the row tables of the new selection are uploaded on a private non-blocking stream and waited for here: host-synchronous
-  // like plan creation, but no device-wide synchronisation through the legacy default stream
+  // host-synchronous like plan creation: waits for the device (the plan's launches in flight), then uploads the row tables
+  // of the new selection on a private stream
+  CK(cudaDeviceSynchronize());   // the old row tables are released below: no launch may still be reading them
   cudaStream_t st = nullptr;
   CK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
   int rc = ERI_OK;

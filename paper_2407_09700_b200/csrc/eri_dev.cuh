@@ -6,7 +6,7 @@
 
 namespace eri {
 
-constexpr int LMAX = 4;
+constexpr int LMAX = 6;   // s..i; tuned kernel families exist up to g, the generic kernels serve h and i
 constexpr double PI = 3.14159265358979323846;
 
 __host__ __device__ constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }
@@ -17,13 +17,13 @@ __host__ __device__ constexpr int nroots_of(int L) { return L / 2 + 1; }  // Eq.
 // Rys data buffer (one device allocation, read-only): see api.cu for how it is filled from rys_tables.inc.
 //   [0..16)    xmax[N]          switch to the Gauss-Hermite asymptote
 //   [16..32)   table offset[N]  (as double)
-//   [32..96)   h_n^2 of the 2N-point Gauss-Hermite rule, N-th block at 32 + N(N-1)/2
-//   [96..160)  v_n, same indexing
-//   [160..)    Chebyshev tables, per N: [interval][k=0..13][2N values]
-constexpr int RYS_HDR_XMAX = 0, RYS_HDR_OFF = 16, RYS_HDR_H2 = 32, RYS_HDR_V = 96, RYS_HDR_SIZE = 160;
+//   [32..128)  h_n^2 of the 2N-point Gauss-Hermite rule, N-th block at 32 + N(N-1)/2   (N <= 13: 91 values)
+//   [128..224) v_n, same indexing
+//   [224..)    Chebyshev tables, per N: [interval][k=0..13][2N values]
+constexpr int RYS_HDR_XMAX = 0, RYS_HDR_OFF = 16, RYS_HDR_H2 = 32, RYS_HDR_V = 128, RYS_HDR_SIZE = 224;
+constexpr int RYS_NROOTS_MAX = 13;   // (ii|ii): floor(24 / 2) + 1; also the gradient of (ii|ih)
 __host__ __device__ constexpr double rys_xmax(int N) {
-  return N == 1 ? 35.0 : N == 2 ? 45.0 : N == 3 ? 50.0 : N == 4 ? 57.5 : N == 5 ? 62.5 : N == 6 ? 67.5
-       : N == 7 ? 72.5 : N == 8 ? 77.5 : 82.5;
+  return N == 1 ? 35.0 : N == 2 ? 45.0 : N == 3 ? 50.0 : 57.5 + 5.0 * (N - 4);   // gen_rys_tables.py XMAX (checked in api.cu)
 }
 __host__ __device__ constexpr int rys_nint(int N) { return (int)(rys_xmax(N) / 2.5 + 0.5); }
 __host__ __device__ constexpr int rys_offset(int N) {  // doubles before the N-th table
@@ -77,7 +77,7 @@ __device__ __forceinline__ void rys_roots(double x, const double* __restrict__ r
 // same interval read the same address (broadcast); the interval stride is padded to 2 (mod 16) doubles, i.e. to 1 (mod 8)
 // 16-byte slots, so that different intervals fall into different slots of a 128-byte wavefront.
 // The buffer holds the layout after the first one, at RYS2_BASE (16-byte aligned).
-constexpr int RYS_TABLE_DOUBLES = 34636;                       // = RYS_TABLE_SIZE of rys_tables.inc (checked in api.cu)
+constexpr int RYS_TABLE_DOUBLES = 83860;                       // = RYS_TABLE_SIZE of rys_tables.inc (checked in api.cu)
 constexpr int RYS2_BASE = RYS_HDR_SIZE + RYS_TABLE_DOUBLES;    // even: 16-byte aligned
 constexpr int RYS2_NMAX = 6;                                   // classes of the thread-per-quartet families have N <= 6
 __host__ __device__ constexpr int rys2_stride(int N) { int s = 28 * N; while (s % 16 != 2) ++s; return s; }

@@ -27,13 +27,13 @@ from multiprocessing import Pool
 
 import mpmath as mp
 
-NMAX = 9
+NMAX = 13   # l <= 6 (h, i functions): N = floor(4*6/2) + 1 = 13 roots for (ii|ii) and for the gradient of (ii|ih)
 WIDTH = 2.5
 DEG = 13
 NCOEF = DEG + 1
 # switch to the Gauss-Hermite asymptote; multiples of WIDTH at or above the smallest x where all 2N moments of
 # the asymptotic rule agree with F_m(x) to 1e-14 relative for every root and weight (verified by check_asymptote below)
-XMAX = {1: 35.0, 2: 45.0, 3: 50.0, 4: 57.5, 5: 62.5, 6: 67.5, 7: 72.5, 8: 77.5, 9: 82.5}
+XMAX = {1: 35.0, 2: 45.0, 3: 50.0, 4: 57.5, 5: 62.5, 6: 67.5, 7: 72.5, 8: 77.5, 9: 82.5, 10: 87.5, 11: 92.5, 12: 97.5, 13: 102.5}
 DPS = 160
 HERE = os.path.dirname(os.path.abspath(__file__))
 

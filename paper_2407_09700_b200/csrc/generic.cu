@@ -10,7 +10,15 @@
 namespace eri {
 namespace {
 
-constexpr int GMAX = 625;  // (l+1)^4 for l = 4
+// Capacity of the per-thread local arrays: LC = 4 serves every input up to g (625 words per axis and root); LC = 6 is the
+// h/i instantiation (2401 words per axis: 58 KB of local memory per thread -- the footprint the paper names as its limit,
+// PAPER.md:151; only launched when a unit really contains an h or i shell).
+template <int LC> struct Cap {
+  static constexpr int G = (LC + 1) * (LC + 1) * (LC + 1) * (LC + 1);        // plain 2-D integrals of one axis
+  static constexpr int G1 = (LC + 2) * (LC + 2) * (LC + 2) * (LC + 1);       // raised on a, b, c (gradient)
+  static constexpr int NM = 2 * LC + 3;                                      // nmax + 1 with both bra indices raised
+  static constexpr int NR = (4 * LC + 1) / 2 + 1;                            // roots, gradient included
+};
 
 struct QuartetGeom {
   double A[3], AB[3], C[3], CD[3];
@@ -25,12 +33,13 @@ struct QuartetGeom {
 // the product centre P (the one with the larger exponent) and transferred to the other one; the opposite order loses
 // up to (|AB|/|PB|)^l digits when a tight and a diffuse function sit several Bohr apart.  swap_bra: build on B,
 // transfer to A with (B-A); c00 must then be given relative to B.  Same for the ket.
+template <int LC>
 __device__ void fill_2d(double* __restrict__ G, int na, int nb, int nc, int nd, double init, double c00, double c00p,
                         double b10, double b01, double b00, double ab, double cd, bool swap_bra, bool swap_ket) {
   const int nmax = na + nb - 2, mmax = nc + nd - 2, M1 = mmax + 1;
-  double T0[11 * 11];   // up to (l+1 raised): nmax, mmax <= 10
-  double tmp[11 * 6];
-  double Bm[6 * 6 * 11];
+  double T0[Cap<LC>::NM * Cap<LC>::NM];   // up to (l+1 raised): nmax, mmax <= 2 LC + 2
+  double tmp[Cap<LC>::NM * (LC + 2)];
+  double Bm[(LC + 2) * (LC + 2) * Cap<LC>::NM];
   T0[0] = init;
   for (int n = 0; n < nmax; ++n) T0[(n + 1) * M1] = c00 * T0[n * M1] + (n > 0 ? n * b10 * T0[(n - 1) * M1] : 0.0);
   for (int m = 0; m < mmax; ++m)
@@ -101,13 +110,13 @@ __device__ __forceinline__ void load_geom(const Work& w, int i, int j, QuartetGe
 
 // Loop over primitive quartets and roots; after the three 2-D integral arrays of a root are ready call
 // cons(gx, gy, gz) -- the weight and all prefactors are folded into gz.
-template <typename Consumer>
+template <int LC, typename Consumer>
 __device__ void quartet_loop(const Work& w, int i, int j, const QuartetGeom& g, Consumer& cons) {
   const PairSet& b = w.bra; const PairSet& k = w.ket;
   const int N = nroots_of(g.la + g.lb + g.lc + g.ld);
   const int na = g.la + 1, nb = g.lb + 1, nc = g.lc + 1, nd = g.ld + 1;
-  double gx[GMAX], gy[GMAX], gz[GMAX];
-  double u[9], wt[9];
+  double gx[Cap<LC>::G], gy[Cap<LC>::G], gz[Cap<LC>::G];
+  double u[Cap<LC>::NR], wt[Cap<LC>::NR];
   for (int kb = 0; kb < b.npp; ++kb) {
     const double p = b.prim[(kb * 5 + 0) * b.stride + i];
     const double P[3] = {b.prim[(kb * 5 + 1) * b.stride + i], b.prim[(kb * 5 + 2) * b.stride + i], b.prim[(kb * 5 + 3) * b.stride + i]};
@@ -131,7 +140,7 @@ __device__ void quartet_loop(const Work& w, int i, int j, const QuartetGeom& g, 
         for (int ax = 0; ax < 3; ++ax) {
           const double c00 = (P[ax] - g.A[ax]) + (swb ? g.AB[ax] : 0.0) - q * t2 * rpq * PQ[ax];
           const double c00p = (Q[ax] - g.C[ax]) + (swk ? g.CD[ax] : 0.0) + p * t2 * rpq * PQ[ax];
-          fill_2d(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax], swb, swk);
+          fill_2d<LC>(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax], swb, swk);
         }
         cons(gx, gy, gz);
       }
@@ -180,22 +189,24 @@ struct StoreConsumer {    // accumulate the Cartesian block [nca][ncb][ncc][ncd]
   }
 };
 
+template <int LC>
 __global__ void __launch_bounds__(128) generic_jk_kernel(Work w) {
   int i, j; double f;
   if (!locate(w, i, j, f)) return;
   QuartetGeom g; load_geom(w, i, j, g);
   DigestConsumer c{w.D, w.J, w.K, w.nao, w.bra.ao[i].x, w.bra.ao[i].y, w.ket.ao[j].x, w.ket.ao[j].y, g.la, g.lb, g.lc, g.ld, f};
-  quartet_loop(w, i, j, g, c);
+  quartet_loop<LC>(w, i, j, g, c);
 }
 
 // list mode only: block t of Cartesian integrals is accumulated at out + off[t] (must be zeroed by the caller)
+template <int LC>
 __global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out, const long long* off) {
   int i, j; double f;
   if (!locate(w, i, j, f)) return;
   const long t = (long)(blockIdx.x * w.nshard + w.shard) * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
   QuartetGeom g; load_geom(w, i, j, g);
   StoreConsumer c{out + off[t], g.la, g.lb, g.lc, g.ld};
-  quartet_loop(w, i, j, g, c);
+  quartet_loop<LC>(w, i, j, g, c);
 }
 
 // ---- gradient (Algorithm 4; Eq. 11) -------------------------------------------
@@ -203,8 +214,7 @@ __global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out,
 // centre and axis; the fourth centre follows from translational invariance.  Per unique quartet
 //   PJ = 4 f D_ab D_cd,  PK = 2 f (D_ac D_bd + D_ad D_bc)
 // and 18 accumulators (3 centres x 3 axes x {J,K}); 24 atomics at the end ("12 atomics per quartet").
-constexpr int GMAX1 = 6 * 6 * 6 * 5;
-
+template <int LC>
 __global__ void __launch_bounds__(128) generic_grad_kernel(Work w) {
   int i, j; double f;
   if (!locate(w, i, j, f)) return;
@@ -216,8 +226,8 @@ __global__ void __launch_bounds__(128) generic_grad_kernel(Work w) {
   const int a0 = b.ao[i].x, b0 = b.ao[i].y, c0 = k.ao[j].x, d0 = k.ao[j].y;
   const int n = w.nao;
   const double* D = w.D;
-  double gx[GMAX1], gy[GMAX1], gz[GMAX1];
-  double u[9], wt[9];
+  double gx[Cap<LC>::G1], gy[Cap<LC>::G1], gz[Cap<LC>::G1];
+  double u[Cap<LC>::NR], wt[Cap<LC>::NR];
   double accJ[9], accK[9];
   for (int x = 0; x < 9; ++x) accJ[x] = accK[x] = 0.0;
   const int Ka = b.npp, Kc = k.npp;
@@ -246,7 +256,7 @@ __global__ void __launch_bounds__(128) generic_grad_kernel(Work w) {
         for (int ax = 0; ax < 3; ++ax) {
           const double c00 = (P[ax] - g.A[ax]) + (swb ? g.AB[ax] : 0.0) - q * t2 * rpq * PQ[ax];
           const double c00p = (Q[ax] - g.C[ax]) + (swk ? g.CD[ax] : 0.0) + p * t2 * rpq * PQ[ax];
-          fill_2d(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax], swb, swk);
+          fill_2d<LC>(G[ax], na, nb, nc, nd, ax == 2 ? pref * wt[r] : 1.0, c00, c00p, b10, b01, b00, g.AB[ax], g.CD[ax], swb, swk);
         }
         const int sa = nb * nc * nd, sb = nc * nd, sc = nd;
         for (int axx = la, ia = 0; axx >= 0; --axx) for (int ay = la - axx; ay >= 0; --ay, ++ia) { const int az = la - axx - ay;
@@ -288,6 +298,8 @@ __global__ void __launch_bounds__(128) generic_grad_kernel(Work w) {
 
 }  // namespace
 
+static bool needs_hi(const Work& w) { return w.bra.la > 4 || w.bra.lb > 4 || w.ket.la > 4 || w.ket.lb > 4; }   // any h or i shell
+
 static int grid_of(const Work& w, int threads, int total_blocks_dense) {
   const int total = w.list ? (w.nlist + threads - 1) / threads : total_blocks_dense;
   return (total + w.nshard - 1) / w.nshard;
@@ -297,7 +309,7 @@ cudaError_t launch_generic_jk(const Work& w, int nblocks_dense, cudaStream_t s) 
   dim3 block(GENERIC_BJ, GENERIC_BI);
   const int grid = grid_of(w, GENERIC_BJ * GENERIC_BI, nblocks_dense);
   if (grid <= 0) return cudaSuccess;
-  generic_jk_kernel<<<grid, block, 0, s>>>(w);
+  if (needs_hi(w)) generic_jk_kernel<6><<<grid, block, 0, s>>>(w); else generic_jk_kernel<4><<<grid, block, 0, s>>>(w);
   return cudaGetLastError();
 }
 
@@ -305,7 +317,7 @@ cudaError_t launch_generic_store(const Work& w, double* out, const long long* of
   dim3 block(GENERIC_BJ, GENERIC_BI);
   const int grid = grid_of(w, GENERIC_BJ * GENERIC_BI, 0);
   if (grid <= 0) return cudaSuccess;
-  generic_store_kernel<<<grid, block, 0, s>>>(w, out, off);
+  if (needs_hi(w)) generic_store_kernel<6><<<grid, block, 0, s>>>(w, out, off); else generic_store_kernel<4><<<grid, block, 0, s>>>(w, out, off);
   return cudaGetLastError();
 }
 
@@ -313,7 +325,7 @@ cudaError_t launch_generic_grad(const Work& w, int nblocks_dense, cudaStream_t s
   dim3 block(GENERIC_GRAD_BJ, GENERIC_GRAD_BI);
   const int grid = grid_of(w, GENERIC_GRAD_BJ * GENERIC_GRAD_BI, nblocks_dense);
   if (grid <= 0) return cudaSuccess;
-  generic_grad_kernel<<<grid, block, 0, s>>>(w);
+  if (needs_hi(w)) generic_grad_kernel<6><<<grid, block, 0, s>>>(w); else generic_grad_kernel<4><<<grid, block, 0, s>>>(w);
   return cudaGetLastError();
 }
 

@@ -31,7 +31,7 @@ cudaError_t launch_coop_grad_class(const Work& w, int nblocks_dense, cudaStream_
 void tuned_catalog(std::vector<std::string>& out);   // "family la lb lc ld" of every tuned instantiation
 
 // transform.cu
-cudaError_t upload_c2s(const double* tables /*host, concatenated ns(l) x nc(l), l = 0..4*/);
+cudaError_t upload_c2s(const double* tables /*host, concatenated ns(l) x nc(l), l = 0..LMAX*/);
 struct ShellMap {          // device arrays describing the AO layout
   const int* sh_l; const int* sh_sph; const int* sh_cart;   // per shell
   const int* sph2sh; const int* cart2sh;                    // per AO

@@ -23,7 +23,7 @@ struct TileGradTraits {
   static constexpr int NLANE = NC * ND + NA * ND + NB * ND;                       // D_cd, D_ad, D_bd: per lane
   static constexpr int STAGE = 32 * 33;
   static constexpr int NE = NA * NB * NC * ND;
-  static constexpr int PERWARP = STAGE + NUNI + 32 * NLANE + (MODE == 3 ? 2 * NE * 32 : 0);   // MODE 3: + the pj, pk columns
+  static constexpr int PERWARP = STAGE + NUNI + 32 * NLANE;
   static constexpr int RT = rys2_size(N);                    // the class's Rys table, first in the block's shared memory
   static constexpr size_t SMEM = sizeof(double) * (RT + BI * PERWARP);
 };
@@ -93,7 +93,7 @@ __device__ __forceinline__ void tile_grad_axis(double* __restrict__ acc, const d
 }
 
 // one differentiated axis of one root with the density products pj[e], pk[e] of the quartet read from a shared-memory column
-// (pjk[32 e], pjk[32 (NE + e)]); accumulates [J: A, B, C | K: A, B, C] of axis AX (MODE 2 and MODE 3)
+// (pjk[32 e], pjk[32 (NE + e)]); accumulates [J: A, B, C | K: A, B, C] of axis AX (MODE 2)
 template <int LA, int LB, int LC, int LD, int AX>
 __device__ __forceinline__ void tile_grad_team_axis(double* __restrict__ acc, const double* c00, const double* c00p, const double* init,
                                                     double b10, double b01, double b00, const double* AB, const double* CD,
@@ -208,18 +208,6 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
 #pragma unroll
       for (int d = 0; d < ND; ++d) Dbd_s[32 * (b * ND + d)] = D[(long)(b0 + b) * n + d0 + d];
     __syncwarp();
-    [[maybe_unused]] double* pjk = mine + 32 * Tr::NLANE;   // MODE 3: pj[e] at 32 e, pk[e] at 32 (NE + e), column of this lane
-    if constexpr (MODE == 3) {
-      // the density products of the row's quartets once, in shared memory: held in registers across the three axis passes they
-      // spilled (profiles/r02_cfg4.md); run-time element index, the loop is short and not unrolled
-#pragma unroll 1
-      for (int e = 0; e < Tr::NE; ++e) {
-        const int d = e % ND, t1 = e / ND, c = t1 % NC, t2 = t1 / NC, b = t2 % NB, a = t2 / NB;
-        pjk[32 * e] = Dab_s[a * NB + b] * Dcd_s[32 * (c * ND + d)];
-        pjk[32 * (Tr::NE + e)] = fma(Dac_s[a * NC + c], Dbd_s[32 * (b * ND + d)], Dad_s[32 * (a * ND + d)] * Dbc_s[b * NC + c]);
-      }
-    }
-
     double acc[18];   // [J: A xyz, B xyz, C xyz | K: same]
 #pragma unroll
     for (int e = 0; e < 18; ++e) acc[e] = 0.0;
@@ -250,27 +238,7 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
           const double hq = 0.5 / q;
           double u[N], wt[N];
           rys_roots_smem<N>(xx, rtab, w.rys, u, wt);
-          if constexpr (MODE == 3) {
-#pragma unroll 1
-            for (int rt = 0; rt < N; ++rt) {
-              const double t2 = u[rt] * rpq;
-              const double b00 = 0.5 * t2, b10 = hp - q * t2 * hp, b01 = hq - p * t2 * hq;
-              const double c00[3] = {(P[0] - A[0]) - q * t2 * PQ[0], (P[1] - A[1]) - q * t2 * PQ[1], (P[2] - A[2]) - q * t2 * PQ[2]};
-              const double c00p[3] = {(Q[0] - C[0]) + p * t2 * PQ[0], (Q[1] - C[1]) + p * t2 * PQ[1], (Q[2] - C[2]) + p * t2 * PQ[2]};
-              const double init[3] = {1.0, 1.0, pref * wt[rt]};
-              double a6[6];
-#pragma unroll
-              for (int ax = 0; ax < 3; ++ax) {
-#pragma unroll
-                for (int e = 0; e < 6; ++e) a6[e] = 0.0;
-                if (ax == 0) tile_grad_team_axis<LA, LB, LC, LD, 0>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
-                else if (ax == 1) tile_grad_team_axis<LA, LB, LC, LD, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
-                else tile_grad_team_axis<LA, LB, LC, LD, 2>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
-#pragma unroll
-                for (int e = 0; e < 6; ++e) acc[(e / 3) * 9 + (e % 3) * 3 + ax] += a6[e];
-              }
-            }
-          } else if constexpr (MODE == 1) {
+          if constexpr (MODE == 1) {
 #pragma unroll 1
             for (int rt = 0; rt < N; ++rt) {
               const double t2 = u[rt] * rpq;

@@ -8,8 +8,9 @@
 namespace eri {
 namespace {
 
-__constant__ double c_c2s[245];   // l-th table at c2s_off(l), ns(l) x nc(l) row-major
-__host__ __device__ constexpr int c2s_off(int l) { return l == 0 ? 0 : l == 1 ? 1 : l == 2 ? 10 : l == 3 ? 40 : 110; }
+__host__ __device__ constexpr int c2s_off(int l) { int off = 0; for (int k = 0; k < l; ++k) off += nsph(k) * ncart(k); return off; }
+constexpr int C2S_SIZE = c2s_off(LMAX + 1);   // 840 doubles for l <= 6
+__constant__ double c_c2s[C2S_SIZE];          // l-th table at c2s_off(l), ns(l) x nc(l) row-major
 
 __global__ void sph2cart_kernel(ShellMap m, const double* __restrict__ Ds, double* __restrict__ Dc) {
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -129,7 +130,7 @@ __global__ void rys_diag_kernel(int N, const double* __restrict__ rys, const dou
                                 double* __restrict__ u, double* __restrict__ w) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
-  double uu[9], ww[9];
+  double uu[RYS_NROOTS_MAX], ww[RYS_NROOTS_MAX];
   rys_roots_rt(N, x[t], rys, uu, ww);
   for (int k = 0; k < N; ++k) { u[(long)t * N + k] = uu[k]; w[(long)t * N + k] = ww[k]; }
 }
@@ -144,7 +145,7 @@ __global__ void rys_diag_smem_kernel(const double* __restrict__ rys, const doubl
   __syncthreads();
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
-  double uu[N], ww[N], u2[9], w2[9];
+  double uu[N], ww[N], u2[RYS_NROOTS_MAX], w2[RYS_NROOTS_MAX];
   rys_roots_smem<N>(x[t], tab, rys, uu, ww);
   rys_roots_rt(N, x[t], rys, u2, w2);
   const double bad = __longlong_as_double(0x7ff8000000000000LL);
@@ -210,7 +211,7 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double* sink, int iters)
 
 }  // namespace
 
-cudaError_t upload_c2s(const double* tables) { return cudaMemcpyToSymbol(c_c2s, tables, sizeof(double) * 245); }
+cudaError_t upload_c2s(const double* tables) { return cudaMemcpyToSymbol(c_c2s, tables, sizeof(double) * C2S_SIZE); }
 
 cudaError_t launch_sph2cart(const ShellMap& m, const double* Ds, double* Dc, cudaStream_t s) {
   const long n2 = (long)m.nao_cart * m.nao_cart;

@@ -36,7 +36,7 @@ def test_every_declared_symbol_is_exported(eri):
 def test_c2s_table_matches_oracle_route(eri):
     """Library: closed formula (reading R3).  Oracle: least-squares projection on scipy's spherical harmonics."""
     import oracle.sph as sph
-    for l in range(5):
+    for l in range(7):
         assert np.abs(eri.eri_c2s_matrix(l) - sph.c2s(l)).max() < 1e-13
 
 
@@ -55,7 +55,7 @@ def test_argument_errors_need_no_device(eri):
     import ctypes
     basis, D, thr = W.cfg0()
     bad = W.Basis(basis.shells.copy(), basis.prims.copy(), basis.coords.copy(), basis.nao)
-    bad.shells["l"][0] = 5
+    bad.shells["l"][0] = 7
     args, keep = eri._basis_args(bad)
     h = ctypes.c_void_p()
     rc = eri.lib().eri_plan_create(*args, ctypes.c_double(0.0), 0, None, ctypes.byref(h))

@@ -47,8 +47,8 @@ def mixed_basis(seed=7, K=2, lmax=4, ncentre=4):
 def test_rys_moment_identity(eri, orc):
     """sum_n w_n u_n^m = F_m(x), m < 2N (definition of the rule) with F_m from the oracle's Boys function."""
     rng = np.random.default_rng(1)
-    for N in range(1, 10):
-        xmax = [0, 35.0, 45.0, 50.0, 57.5, 62.5, 67.5, 72.5, 77.5, 82.5][N]
+    for N in range(1, 14):
+        xmax = [0, 35.0, 45.0, 50.0, 57.5, 62.5, 67.5, 72.5, 77.5, 82.5, 87.5, 92.5, 97.5, 102.5][N]
         xs = np.concatenate([rng.uniform(0, xmax, 200), [0.0, 1e-12, 2.5 - 1e-12, 2.5, 2.5 + 1e-12, xmax - 1e-9, xmax, xmax + 1e-9],
                              np.exp(rng.uniform(math.log(xmax), math.log(5e4), 50))])
         u, w = eri.eri_rys_roots(N, xs)
@@ -101,7 +101,7 @@ def test_schwarz_matches_oracle(eri, orc):
 
 def test_c2s_table_matches_oracle(eri):
     import oracle.sph as sph
-    for l in range(5):
+    for l in range(7):
         assert np.abs(eri.eri_c2s_matrix(l) - sph.c2s(l)).max() < 1e-13
 
 
@@ -286,6 +286,56 @@ def test_grad_finite_difference_of_gpu_energy(eri):
         assert abs(fdK - gK[atom, ax].item()) <= 1e-6 * scale
 
 
+# ----------------------------------------------------------------------------------------------- h and i functions
+def hi_basis(seed=41, ncentre=3):
+    """shells l = 0..6 (s..i) spread over `ncentre` centres in a 3 Bohr box, one primitive each, two for p and h"""
+    rng = np.random.default_rng(seed)
+    coords = rng.uniform(0.0, 3.0, (ncentre, 3))
+    atom_shells = [[] for _ in range(ncentre)]
+    for l in range(7):
+        K = 2 if l in (1, 5) else 1
+        e = np.sort(np.exp(rng.uniform(math.log(0.4), math.log(2.5), K)))[::-1].copy()
+        atom_shells[l % ncentre].append((l, e, W.normalise(l, e, rng.uniform(0.3, 1.0, K))))
+    return W._assemble(atom_shells, coords, {"name": "hi"})
+
+
+def test_eri_blocks_with_h_and_i_shells(eri, orc):
+    """The paper stops at g because its 2-D integrals overflow per-thread local memory; here l = 5, 6 run on the
+    generic kernels (N up to 13 roots) and must match the oracle like every other class."""
+    basis = hi_basis()
+    ls = basis.shells["l"]
+    h, i6 = int(np.where(ls == 5)[0][0]), int(np.where(ls == 6)[0][0])
+    quartets = [(h, 0, 0, 0), (i6, 0, 0, 0), (h, 1, 2, 0), (i6, 2, 1, 1), (h, h, 0, 0), (i6, 3, h, 1), (h, i6, 4, 2), (i6, i6, 0, 0),
+                (0, h, i6, 1), (i6, h, i6, h), (h, h, h, h)]
+    got = eri.eri_compute_quartets(basis, quartets)
+    ref = [orc.eri_block(basis, *q) for q in quartets]
+    for q, a, r in zip(quartets, got, ref):
+        assert np.abs(a - r).max() <= 1e-11 * max(np.abs(r).max(), 1e-3), (q, [int(ls[s]) for s in q])
+
+
+def test_jk_and_gradient_with_h_and_i_shells(eri, orc):
+    basis = hi_basis(seed=43)
+    rng = np.random.default_rng(6)
+    C = rng.standard_normal((basis.nao, 6)) / math.sqrt(basis.nao)
+    D = C @ C.T
+    _jk_parity(eri, orc, basis, D, 0.0)
+    # explicit lists of h/i classes (cfg1 recipe)
+    ls = basis.shells["l"]
+    h, i6, s0, p1 = (int(np.where(ls == l)[0][0]) for l in (5, 6, 0, 1))
+    q = np.array([(h, s0, s0, s0), (i6, p1, h, s0), (i6, i6, s0, s0), (h, h, p1, p1)], dtype=np.int32)
+    Jt, Kt = eri.eri_digest_quartet_list(basis, q, dev(D))
+    Jo, Ko = orc.digest_list(basis, D, q)
+    scale = max(np.abs(Jo).max(), np.abs(Ko).max())
+    assert np.abs(Jt.cpu().numpy() - Jo).max() <= JK_TOL * scale and np.abs(Kt.cpu().numpy() - Ko).max() <= JK_TOL * scale
+    # gradient: a smaller set (s, p, h, i on three centres) keeps the oracle to seconds
+    keep = np.isin(ls, (0, 1, 5, 6))
+    sub = W._assemble([[(int(basis.shells["l"][s]), basis.prims["exp"][basis.shells["prim_off"][s]:basis.shells["prim_off"][s] + basis.shells["nprim"][s]],
+                         basis.prims["coef"][basis.shells["prim_off"][s]:basis.shells["prim_off"][s] + basis.shells["nprim"][s]])
+                        for s in range(basis.nshell) if keep[s] and basis.shells["atom"][s] == a] for a in range(basis.natm)], basis.coords, {})
+    C = rng.standard_normal((sub.nao, 5)) / math.sqrt(sub.nao)
+    _grad_parity(eri, orc, sub, C @ C.T, 0.0)
+
+
 # ----------------------------------------------------------------------------------------------- edge cases
 def test_edge_cases(eri, orc):
     basis, D, thr = W.cfg0()
@@ -301,7 +351,7 @@ def test_edge_cases(eri, orc):
     assert eri.eri_compute_quartets(basis, np.zeros((0, 4), dtype=np.int32)) == []
     # error paths
     bad = W.Basis(basis.shells.copy(), basis.prims.copy(), basis.coords.copy(), basis.nao)
-    bad.shells["l"][0] = 5
+    bad.shells["l"][0] = 7
     with pytest.raises(eri.EriError, match="angular momentum"):
         eri.eri_plan_create(bad, 0.0)
     bad.shells["l"][0] = 0

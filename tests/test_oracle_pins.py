@@ -22,27 +22,27 @@ from quadrature_ref import cart_powers, prim_block_quadrature, prim_eri_quadratu
 
 # ------------------------------------------------------------------------------------------------ Boys
 def test_boys_at_zero(orc):
-    F = orc.boys(17, 0.0)
-    assert np.allclose(F, [1.0 / (2 * m + 1) for m in range(18)], rtol=1e-15)
+    F = orc.boys(25, 0.0)
+    assert np.allclose(F, [1.0 / (2 * m + 1) for m in range(26)], rtol=1e-15)
 
 
 @pytest.mark.parametrize("x", [1e-8, 1e-3, 0.3, 1.0, 4.7, 12.0, 25.0, 34.999, 35.0, 35.001, 50.0, 90.0, 150.0])
 def test_boys_incomplete_gamma_and_recursion(orc, x):
-    F = orc.boys(17, x)
+    F = orc.boys(25, x)       # m up to 25: (ii|ii) with one raised index
     assert F[0] == pytest.approx(0.5 * math.sqrt(math.pi / x) * erf(math.sqrt(x)), rel=2e-15)
-    for m in range(18):
+    for m in range(26):
         ref = gamma(m + 0.5) * gammainc(m + 0.5, x) / (2.0 * x ** (m + 0.5))
         if x >= 1e-3:  # gammainc loses relative accuracy for tiny x; covered by the mpmath test
             assert F[m] == pytest.approx(ref, rel=5e-14)
-    for m in range(17):  # (2m+1) F_m = 2x F_{m+1} + e^-x
+    for m in range(25):  # (2m+1) F_m = 2x F_{m+1} + e^-x
         assert (2 * m + 1) * F[m] == pytest.approx(2 * x * F[m + 1] + math.exp(-x), rel=1e-13)
 
 
 @pytest.mark.parametrize("x", [1e-8, 0.02, 2.5, 18.0, 33.0, 36.0, 71.0])
 def test_boys_mpmath_quadrature(orc, x):
     mpmath.mp.dps = 30
-    F = orc.boys(17, x)
-    for m in (0, 1, 5, 9, 16, 17):
+    F = orc.boys(25, x)
+    for m in (0, 1, 5, 9, 16, 17, 21, 25):
         ref = mpmath.quad(lambda t: t ** (2 * m) * mpmath.exp(-x * t * t), [0, 1])
         assert F[m] == pytest.approx(float(ref), rel=1e-14)
 
@@ -88,7 +88,8 @@ def _rand_powers(rng, l):
 
 @pytest.mark.parametrize("ls", [(1, 0, 0, 0), (1, 1, 0, 0), (1, 0, 1, 0), (1, 1, 1, 1), (2, 0, 0, 0), (2, 1, 1, 0), (2, 2, 1, 1),
                                 (2, 2, 2, 2), (3, 0, 2, 1), (3, 3, 1, 0), (3, 3, 3, 3), (4, 0, 0, 0), (4, 2, 3, 1),
-                                (4, 4, 2, 2), (4, 4, 4, 4), (0, 2, 0, 3), (1, 4, 2, 4)])
+                                (4, 4, 2, 2), (4, 4, 4, 4), (0, 2, 0, 3), (1, 4, 2, 4),
+                                (5, 0, 0, 0), (6, 0, 1, 0), (5, 5, 0, 0), (6, 2, 5, 1), (6, 6, 6, 6)])
 def test_primitive_eri_vs_bruteforce_quadrature(orc, ls):
     rng = np.random.default_rng(100 + sum(ls) * 7 + ls[0])
     for _ in range(3):
@@ -137,7 +138,7 @@ def test_c2s_explicit_low_l(orc):
     assert np.allclose(sph.c2s(2), ref, atol=1e-13)
 
 
-@pytest.mark.parametrize("l", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("l", [0, 1, 2, 3, 4, 5, 6])
 def test_c2s_harmonic_orthonormal(orc, l):
     from oracle import sph
     T = sph.c2s(l)
@@ -206,7 +207,7 @@ def test_block_quadrature_matches_component_quadrature():
 
 
 @pytest.mark.parametrize("ls,ks", [((1, 2, 3, 0), (2, 1, 1, 2)), ((2, 2, 1, 1), (1, 2, 2, 1)), ((4, 0, 1, 0), (2, 1, 2, 1)),
-                                   ((0, 3, 2, 1), (2, 2, 1, 1))])
+                                   ((0, 3, 2, 1), (2, 2, 1, 1)), ((5, 0, 1, 0), (1, 1, 2, 1)), ((1, 6, 0, 0), (2, 1, 1, 1))])
 def test_contracted_spherical_block_vs_quadrature(orc, ls, ks):
     """The oracle's contraction (Eq. 5) and its four-index Cartesian -> spherical transform (reading R3) for
     l >= 1: expected block = einsum of brute-force quadrature primitive blocks with the RAW coefficients and the c2s
@@ -232,7 +233,7 @@ def test_contracted_spherical_block_vs_quadrature(orc, ls, ks):
     assert np.abs(val - ref).max() <= 1e-11 * np.abs(ref).max()
 
 
-@pytest.mark.parametrize("l", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("l", [0, 1, 2, 3, 4, 5, 6])
 def test_contracted_spherical_shells_are_orthonormal(orc, l):
     """SURVEY 8(c) "c2s matrices" pin: a contracted shell normalised by reading R2 has unit self-overlap and its 2l+1
     functions are orthonormal; the overlap comes from the oracle's E_0 Hermite coefficients, S = E0x E0y E0z (pi/p)^(3/2),
@@ -241,7 +242,7 @@ def test_contracted_spherical_shells_are_orthonormal(orc, l):
     rng = np.random.default_rng(900 + l)
     e = np.exp(rng.uniform(-1.5, 2.5, 3))
     c = W.normalise(l, e, rng.uniform(0.2, 1.0, 3))
-    l2 = (l + 2) % 5
+    l2 = (l + 2) % 7
     e2 = np.exp(rng.uniform(-1.0, 1.0, 2))
     c2 = W.normalise(l2, e2, rng.uniform(0.2, 1.0, 2))
     ctr = rng.uniform(-1, 1, 3)
