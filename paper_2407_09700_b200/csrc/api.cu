@@ -7,12 +7,14 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <deque>
 #include <map>
 #include <memory>
 #include <mutex>
 #include <new>
 #include <set>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/eri.h"
@@ -81,10 +83,14 @@ struct Dev {   // owning device array
     n = count;
     return cudaStreamSynchronize(as);
   }
-  cudaError_t upload(const std::vector<T>& h, cudaStream_t s) {
+  // the copy runs on the allocator's private stream and is complete on return: the data can then be used on any stream, and
+  // uploads never wait for (or serialise with) kernels queued on the caller's stream, e.g. the Schwarz pass of plan creation
+  cudaError_t upload(const std::vector<T>& h, cudaStream_t /*unused*/) {
     cudaError_t e = alloc(h.size());
     if (e != cudaSuccess || h.empty()) return e;
-    return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+    e = cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, g_alloc_stream);
+    if (e != cudaSuccess) return e;
+    return cudaStreamSynchronize(g_alloc_stream);
   }
 };
 
@@ -169,6 +175,27 @@ int ensure_init() {
   return ERI_OK;
 }
 
+// Host loops of plan creation over a few worker threads (pair records, work units): contiguous ranges, the workers bind to the
+// library's device first (a new host thread starts on device 0).  f(lo, hi) returns an eri error code; the first failure wins.
+template <class F>
+int parallel_ranges(int n, int min_per_thread, F f) {
+  const int hw = (int)std::thread::hardware_concurrency();
+  const int nt = std::max(1, std::min(std::min(hw > 0 ? hw : 4, 16), n / std::max(1, min_per_thread)));
+  if (nt <= 1) return f(0, n);
+  std::vector<int> rc(nt, ERI_OK);
+  std::vector<std::string> msg(nt);
+  std::vector<std::thread> th;
+  for (int t = 0; t < nt; ++t)
+    th.emplace_back([&, t] {
+      if (g_device >= 0) cudaSetDevice(g_device);
+      rc[t] = f((int)((long long)n * t / nt), (int)((long long)n * (t + 1) / nt));
+      if (rc[t] != ERI_OK) msg[t] = g_err;
+    });
+  for (auto& x : th) x.join();
+  for (int t = 0; t < nt; ++t) if (rc[t] != ERI_OK) { g_err = msg[t]; return rc[t]; }
+  return ERI_OK;
+}
+
 // ---- basis ----------------------------------------------------------------------------------------------------
 struct Group { int l, K; std::vector<int> shells; };
 
@@ -237,7 +264,8 @@ int upload_pair_class(const Basis& b, PairClass& pc, cudaStream_t s) {
   std::vector<double> prim((size_t)pc.npp * 5 * st, 0.0), geom(7 * st, 0.0), aexp((size_t)pc.npp * 2 * st, 0.0), q(st, 0.0);
   std::vector<int2> ao(st, make_int2(0, 0)), atom(st, make_int2(0, 0));
   const double kfac = std::sqrt(2.0) * std::pow(PI, 1.25);
-  for (int i = 0; i < n; ++i) {
+  parallel_ranges(n, std::max(1, 16384 / pc.npp), [&](int lo_i, int hi_i) {
+  for (int i = lo_i; i < hi_i; ++i) {
     const eri_shell_t& A = b.sh[pc.sa[i]]; const eri_shell_t& B = b.sh[pc.sb[i]];
     const double* RA = &b.xyz[3 * A.atom]; const double* RB = &b.xyz[3 * B.atom];
     const double ab[3] = {RA[0] - RB[0], RA[1] - RB[1], RA[2] - RB[2]};
@@ -259,9 +287,9 @@ int upload_pair_class(const Basis& b, PairClass& pc, cudaStream_t s) {
         aexp[((size_t)k * 2 + 0) * st + i] = ea; aexp[((size_t)k * 2 + 1) * st + i] = eb;
       }
   }
+  return (int)ERI_OK; });
   CK(pc.prim.upload(prim, s)); CK(pc.geom.upload(geom, s)); CK(pc.aexp.upload(aexp, s)); CK(pc.q.upload(q, s));
-  CK(pc.ao.upload(ao, s)); CK(pc.atom.upload(atom, s));
-  CK(cudaStreamSynchronize(s));   // the host vectors die here
+  CK(pc.ao.upload(ao, s)); CK(pc.atom.upload(atom, s));   // complete on return (Dev::upload)
   return ERI_OK;
 }
 
@@ -320,26 +348,34 @@ void init_pair_class(const Basis& b, int ga, int gb, PairClass& pc) {
 }
 
 // Schwarz factors of every pair of pc (Eq. 7) through the generic store kernel on the quartets (ab|ab).
-int schwarz_of_class(PairClass& pc, cudaStream_t s) {
+// Enqueue only: the Cartesian blocks go to a scratch buffer that all classes share (stream order keeps them apart), the
+// factors to a device array of the class; schwarz_collect copies them to the host after ONE synchronisation for all classes
+// (a synchronisation per class and chunk was a good part of plan creation, profiles/r02_plan.md).
+struct SchwarzScratch {
+  Dev<double> cart; Dev<int2> list; Dev<long long> off;
+  size_t cart_cap = 0, list_cap = 0;
+};
+int schwarz_enqueue(PairClass& pc, Dev<double>& qdev, SchwarzScratch& sc, cudaStream_t s) {
   const int n = pc.npair;
   pc.Q.assign(n, 0.0);
   if (n == 0) return ERI_OK;
   const long nab = (long)ncart(pc.la) * ncart(pc.lb), blk = nab * nab;
   const int chunk = (int)std::max<long>(1, std::min<long>(n, (64L << 20) / blk));
-  Dev<double> cart, qd; Dev<int2> list; Dev<long long> off;
-  CK(cart.alloc((size_t)chunk * blk)); CK(qd.alloc(chunk));
-  std::vector<int2> hl(chunk); std::vector<long long> ho(chunk);
+  if (sc.cart_cap < (size_t)chunk * blk) { CK(cudaStreamSynchronize(s)); sc.cart_cap = (size_t)chunk * blk; CK(sc.cart.alloc(sc.cart_cap)); }
+  if (sc.list_cap < (size_t)chunk) { CK(cudaStreamSynchronize(s)); sc.list_cap = chunk; CK(sc.list.alloc(chunk)); CK(sc.off.alloc(chunk)); }
+  CK(qdev.alloc(n));
   for (int start = 0; start < n; start += chunk) {
     const int m = std::min(chunk, n - start);
-    for (int t = 0; t < m; ++t) { hl[t] = make_int2(start + t, start + t); ho[t] = (long long)t * blk; }
-    CK(list.upload(hl, s)); CK(off.upload(ho, s));
-    CK(cudaMemsetAsync(cart.p, 0, sizeof(double) * (size_t)m * blk, s));
-    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = list.p; w.nlist = m; w.rys = g_rys; w.nshard = 1;
-    CK(launch_generic_store(w, cart.p, off.p, s));
-    CK(launch_schwarz_diag(pc.la, pc.lb, m, cart.p, qd.p, s));
-    CK(cudaMemcpyAsync(pc.Q.data() + start, qd.p, sizeof(double) * m, cudaMemcpyDeviceToHost, s));
-    CK(cudaStreamSynchronize(s));
+    CK(launch_diag_list(sc.list.p, sc.off.p, start, m, s));
+    CK(cudaMemsetAsync(sc.cart.p, 0, sizeof(double) * (size_t)m * blk, s));
+    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = sc.list.p; w.nlist = m; w.rys = g_rys; w.nshard = 1;
+    CK(launch_generic_store(w, sc.cart.p, sc.off.p, m, s));   // element-major blocks: coalesced accumulation
+    CK(launch_schwarz_diag(pc.la, pc.lb, m, sc.cart.p, qdev.p + start, s));
   }
+  return ERI_OK;
+}
+int schwarz_collect(PairClass& pc, Dev<double>& qdev) {   // after the stream has been synchronised
+  if (pc.npair) CK(cudaMemcpy(pc.Q.data(), qdev.p, sizeof(double) * pc.npair, cudaMemcpyDeviceToHost));
   return ERI_OK;
 }
 
@@ -487,9 +523,12 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
         if (lo == 0) continue;
         slot.push_back(HALF * hb); off.push_back(off.back() + lo);
         // lane slots actually swept = rows with work x 32 (the kernel skips the other rows; rows are sorted within the half)
+        // rows of the half and ket chunks are both sorted by decreasing factor: the number of rows with work can only
+        // shrink from one chunk to the next (two-pointer sweep instead of a scan of the 16 rows per chunk)
+        int nr = 0;
+        while (nr < HALF && gb.Q[HALF * hb + nr] >= 0.0) ++nr;
         for (int ck = 0; ck < lo; ++ck) {
-          int nr = 0;
-          while (nr < HALF && gb.Q[HALF * hb + nr] >= 0.0 && gb.Q[HALF * hb + nr] * gk.half_q[2 * ck] >= pl.thr) ++nr;
+          while (nr > 0 && gb.Q[HALF * hb + nr - 1] * gk.half_q[2 * ck] < pl.thr) --nr;
           slots += 32 * nr;
         }
       }
@@ -648,6 +687,8 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
   pl.stats.plan_ms_init = lap();
   // pair sets |ab, KaKb} for group(a) >= group(b) (groups sorted by (l,K), so la >= lb) -- Alg. 1 lines 3-6
   std::vector<std::unique_ptr<PairClass>> all;
+  std::deque<Dev<double>> qdev;   // Schwarz factors of the classes on the device until the one synchronisation below
+  SchwarzScratch scratch;
   double qmax = 0.0;
   long long pairs_total = 0;
   for (int ga = 0; ga < ng; ++ga)
@@ -661,10 +702,16 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
         }
       pairs_total += (long long)pc->sa.size();
       CKI(upload_pair_class(b, *pc, s));
-      CKI(schwarz_of_class(*pc, s));
-      for (double q : pc->Q) qmax = std::max(qmax, q);
+      qdev.emplace_back();
+      CKI(schwarz_enqueue(*pc, qdev.back(), scratch, s));
       all.push_back(std::move(pc));
     }
+  CK(cudaStreamSynchronize(s));
+  for (size_t k = 0; k < all.size(); ++k) {
+    CKI(schwarz_collect(*all[k], qdev[k]));
+    for (double q : all[k]->Q) qmax = std::max(qmax, q);
+  }
+  qdev.clear();
   pl.stats.plan_ms_schwarz = lap();
   // prescreen (Alg. 1 line 7), sort by decreasing bound (the paper bins, Eq. 6; sorting is the limit of fine bins)
   long long pairs_kept = 0;
@@ -690,8 +737,12 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
   pl.stats.plan_ms_pairs = lap();
   // work units: bra set P >= ket set R; per bra pair the kept kets are a prefix of the sorted ket set (reading R7)
   long long qkept = 0; double flops = 0, flops_g = 0;
-  for (int P = 0; P < (int)pl.pcs.size(); ++P)
-    for (int R = 0; R <= P; ++R) {
+  std::vector<std::pair<int, int>> cand;
+  for (int P = 0; P < (int)pl.pcs.size(); ++P) for (int R = 0; R <= P; ++R) cand.push_back({P, R});
+  std::vector<std::unique_ptr<Unit>> built(cand.size());
+  CKI(parallel_ranges((int)cand.size(), 8, [&](int lo_u, int hi_u) {
+    for (int c = lo_u; c < hi_u; ++c) {
+      const int P = cand[c].first, R = cand[c].second;
       const PairClass& bp = *pl.pcs[P]; const PairClass& kp = *pl.pcs[R];
       auto u = std::make_unique<Unit>();
       u->P = P; u->R = R; u->same = (P == R);
@@ -713,10 +764,16 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
       u->flops_grad = tot * canonical_flops(bp.la, bp.lb, kp.la, kp.lb, bp.Ka, bp.Kb, kp.Ka, kp.Kb, 1);
       CK(u->ket_count.upload(u->h_count, s));
       CKI(select_kernels(pl, *u, s));
-      qkept += tot; flops += u->flops; flops_g += u->flops_grad;
-      u->index = (int)pl.units.size();
-      pl.units.push_back(std::move(u));
+      built[c] = std::move(u);
     }
+    return (int)ERI_OK;
+  }));
+  for (auto& u : built) {
+    if (!u) continue;
+    qkept += u->quartets; flops += u->flops; flops_g += u->flops_grad;
+    u->index = (int)pl.units.size();
+    pl.units.push_back(std::move(u));
+  }
   CK(cudaStreamSynchronize(s));
   pl.stats.plan_ms_units = lap();
   eri_stats_t& st = pl.stats;
@@ -1100,7 +1157,7 @@ int eri_compute_quartets(const eri_shell_t* shells, int nshell, const eri_prim_t
     CK(cudaMemsetAsync(cart.p, 0, sizeof(double) * (size_t)ctot, s));
     for (auto& up : pl.units) {
       Work w = make_work(pl, *up, false);
-      CK(launch_generic_store(w, cart.p, up->coff.p, s));
+      CK(launch_generic_store(w, cart.p, up->coff.p, 1, s));
     }
     std::vector<int> q4(quartets, quartets + 4 * (size_t)n);
     std::vector<long long> ooff(out_off, out_off + n);
@@ -1126,7 +1183,10 @@ int eri_schwarz(const eri_shell_t* shells, int nshell, const eri_prim_t* prims, 
         PairClass pc; init_pair_class(b, ga, gb, pc);
         for (int A : b.groups[ga].shells) for (int B : b.groups[gb].shells) { pc.sa.push_back(A); pc.sb.push_back(B); }
         CKI(upload_pair_class(b, pc, s));
-        CKI(schwarz_of_class(pc, s));
+        Dev<double> qd; SchwarzScratch sc;
+        CKI(schwarz_enqueue(pc, qd, sc, s));
+        CK(cudaStreamSynchronize(s));
+        CKI(schwarz_collect(pc, qd));
         for (int i = 0; i < pc.npair; ++i) Q[(size_t)pc.sa[i] * nshell + pc.sb[i]] = Q[(size_t)pc.sb[i] * nshell + pc.sa[i]] = pc.Q[i];
       }
     return ERI_OK;

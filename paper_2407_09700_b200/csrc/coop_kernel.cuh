@@ -93,6 +93,63 @@ __device__ __forceinline__ void fill_2d_smem(double* __restrict__ dst, int s1, i
   }
 }
 
+// Phase 1 in two stages for the eight-warp class (gg|gg).  With one lane per (root, axis) the 27 lanes that build the 2-D
+// integrals work alone while the other 229 wait, and that build -- mostly the ket transfer, 25 values for each of the 25 bra
+// index pairs -- is as long as the product phase.  Stage a: lane (root, axis) runs the vertical recurrence and the bra
+// transfer and leaves B(i1, i2, m), m = 0..l3+l4, in a scratch area; stage b: the 3 N (l1+1)(l2+1) independent ket transfers
+// are dealt over all lanes of the group.  Measured on cfg1 (profiles/r02_cfg1.md): (gg|gg) K = 3 2174 -> 1801 ms (15.8 -> 19.2 %
+// of the FP64 peak), K = 1 100.9 -> 93.7 ms; for the four-warp classes the extra shared memory (one block per SM instead of two
+// for (gg|gf), (gf|gf): 1530 -> 2345 ms) and the second barrier cost more than the idle lanes, so they keep the one-stage build.
+template <int L1, int L2, int MM>
+__device__ __forceinline__ void fill_2d_bra(double* __restrict__ scr, double init, double c00, double c00p, double b10, double b01,
+                                            double b00, double x12) {
+  constexpr int NM = L1 + L2;
+  double T[NM + 1][MM + 1];
+  T[0][0] = init;
+#pragma unroll
+  for (int n = 0; n < NM; ++n) T[n + 1][0] = n > 0 ? fma(c00, T[n][0], (n * b10) * T[n - 1][0]) : c00 * T[n][0];
+#pragma unroll
+  for (int m = 0; m < MM; ++m)
+#pragma unroll
+    for (int n = 0; n <= NM; ++n) {
+      double v = c00p * T[n][m];
+      if (m > 0) v = fma(m * b01, T[n][m - 1], v);
+      if (n > 0) v = fma(n * b00, T[n - 1][m], v);
+      T[n][m + 1] = v;
+    }
+#pragma unroll
+  for (int j = 0; j <= L2; ++j) {
+    if (j > 0) {
+#pragma unroll
+      for (int i = 0; i <= NM - j; ++i)
+#pragma unroll
+        for (int m = 0; m <= MM; ++m) T[i][m] = fma(x12, T[i][m], T[i + 1][m]);
+    }
+#pragma unroll
+    for (int i = 0; i <= L1; ++i)
+#pragma unroll
+      for (int m = 0; m <= MM; ++m) scr[(i * (L2 + 1) + j) * (MM + 1) + m] = T[i][m];
+  }
+}
+
+// one ket transfer: R(m) = B(i1, i2, m) -> I(i1, i2, i3, i4) at dst[i3 * s3 + i4 * s4]
+template <int L3, int L4>
+__device__ __forceinline__ void ket_transfer(const double* __restrict__ src, double* __restrict__ dst, int s3, int s4, double x34) {
+  constexpr int MM = L3 + L4;
+  double R[MM + 1];
+#pragma unroll
+  for (int m = 0; m <= MM; ++m) R[m] = src[m];
+#pragma unroll
+  for (int l = 0; l <= L4; ++l) {
+    if (l > 0) {
+#pragma unroll
+      for (int k = 0; k <= MM - l; ++k) R[k] = fma(x34, R[k], R[k + 1]);
+    }
+#pragma unroll
+    for (int k = 0; k <= L3; ++k) dst[k * s3 + l * s4] = R[k];
+  }
+}
+
 __device__ __forceinline__ void cart_powers(int l, int k, int& lx, int& ly, int& lz) {
   int row = 0;
   while ((row + 1) * (row + 2) / 2 <= k) ++row;   // row = l - lx
@@ -126,8 +183,12 @@ struct CoopTraits {
   static constexpr int SLAB2D = 3 * N * G2;
   static constexpr int KROW = (2 * (NC + ND)) | 1;           // per (a,b): Kac[NC] Kad[ND] Kbc[NC] Kbd[ND]; odd stride: no bank conflicts
   static constexpr int SLABK = PASSES * T * KROW;
-  static constexpr int SLAB = (SLAB2D > SLABK ? SLAB2D : SLABK) + NCD;   // + staged D_cd
+  static constexpr bool SPLIT1 = TW >= 8;                    // two-stage phase 1 (fill_2d_bra + ket_transfer): the slab-bound class (gg|gg)
+  static constexpr int NIJ = (LA + 1) * (LB + 1), MM1 = LC + LD + 1;
+  static constexpr int SCR = SPLIT1 ? 3 * N * NIJ * MM1 : 0;    // B(i, j, m) of every (root, axis)
+  static constexpr int SLAB = (SLAB2D > SLABK ? SLAB2D : SLABK) + SCR + NCD;   // + bra-transfer scratch + staged D_cd
   static constexpr size_t SMEM = sizeof(double) * SLAB * GROUPS;
+  static_assert(SMEM <= 227 * 1024, "cooperative kernel: shared memory");
 };
 
 template <int LA, int LB, int LC, int LD, int TW, int NCH = 1>
@@ -140,6 +201,7 @@ __global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WAR
   const int lane = threadIdx.x, wy = threadIdx.y;   // lane: thread within the group of T; wy: group within the block
   double* S = smem + (size_t)wy * Tr::SLAB;      // 2-D integrals, later the K partial sums
   double* sDcd = S + (Tr::SLAB - NCD);             // D_cd of the task's ket pair
+  [[maybe_unused]] double* scr = S + (Tr::SLAB - NCD - Tr::SCR);   // two-stage phase 1: B(i, j, m) per (root, axis)
 
   const PairSet& bp = w.bra; const PairSet& kp = w.ket;
   const int blk = blockIdx.x * w.nshard + w.shard;
@@ -245,6 +307,42 @@ __global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WAR
         const double PQ[3] = {P[0] - Q[0], P[1] - Q[1], P[2] - Q[2]};
         const double x = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
         // ---- phase 1 ----
+        if constexpr (Tr::SPLIT1) {
+          constexpr int NIJ = Tr::NIJ, MM1 = Tr::MM1;
+          constexpr int SI = (LB + 1) * SCD, SJ = SCD, SK = LD + 1, SL = 1;
+          const double cdx3[3] = {CD[0], CD[1], CD[2]};
+          if (fill_lane) {   // stage a: vertical recurrence + bra transfer
+            double u, wt;
+            rys_root_one<N>(x, w.rys, my_root, u, wt);
+            const double t2 = u * rpq;
+            const double b00 = 0.5 * t2, b10 = (1.0 - q * t2) * 0.5 / p, b01 = (1.0 - p * t2) * 0.5 / q;
+            const int ax = my_axis;
+            const double pa = (ax == 0 ? P[0] - A[0] : ax == 1 ? P[1] - A[1] : P[2] - A[2]);
+            const double qc = (ax == 0 ? Q[0] - C[0] : ax == 1 ? Q[1] - C[1] : Q[2] - C[2]);
+            const double pqx = (ax == 0 ? PQ[0] : ax == 1 ? PQ[1] : PQ[2]);
+            const double abx = (ax == 0 ? AB[0] : ax == 1 ? AB[1] : AB[2]);
+            const double cdx = cdx3[ax];
+            const double c00 = pa + (swb ? abx : 0.0) - q * t2 * pqx;
+            const double c00p = qc + (swk ? cdx : 0.0) + p * t2 * pqx;
+            const double init = ax == 2 ? Kab * Kcd * sqrt(rpq) * wt : 1.0;
+            double* dsts = scr + (ax * N + my_root) * (NIJ * MM1);   // B(i1, i2, m): i1 on the build centre
+            if (!swb) fill_2d_bra<LA, LB, LC + LD>(dsts, init, c00, c00p, b10, b01, b00, abx);
+            else if constexpr (LB > 0) fill_2d_bra<LB, LA, LC + LD>(dsts, init, c00, c00p, b10, b01, b00, -abx);
+          }
+          group_sync(TW, wy);
+          // stage b: ket transfers, one per (root, axis, i1, i2), over all lanes of the group
+          for (int tk = lane; tk < 3 * N * NIJ; tk += T) {
+            const int ra = tk / NIJ, ij = tk - ra * NIJ, ax = ra / N;   // ra = axis * N + root
+            const double* src = scr + (size_t)tk * MM1;
+            // (i1, i2) -> (i, j) of the slab: built on A: i1 = i, i2 = j; built on B: i1 = j, i2 = i
+            int i1, i2, off;
+            if (!swb) { i1 = ij / (LB + 1); i2 = ij - i1 * (LB + 1); off = i1 * SI + i2 * SJ; }
+            else      { i1 = ij / (LA + 1); i2 = ij - i1 * (LA + 1); off = i2 * SI + i1 * SJ; }
+            double* dst = S + ra * G2 + off;
+            if (!swk) ket_transfer<LC, LD>(src, dst, SK, SL, cdx3[ax]);
+            else if constexpr (LD > 0) ket_transfer<LD, LC>(src, dst, SL, SK, -cdx3[ax]);
+          }
+        } else
         if (fill_lane) {
           double u, wt;
           rys_root_one<N>(x, w.rys, my_root, u, wt);

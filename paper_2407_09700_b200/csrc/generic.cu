@@ -174,8 +174,8 @@ struct DigestConsumer {   // six updates of Alg. 2 lines 8-13
   }
 };
 
-struct StoreConsumer {    // accumulate the Cartesian block [nca][ncb][ncc][ncd]; one thread owns the block
-  double* out; int la, lb, lc, ld;
+struct StoreConsumer {    // accumulate the Cartesian block [nca][ncb][ncc][ncd] (element e at out[e * stride]); one thread owns the block
+  double* out; int la, lb, lc, ld; long stride;
   __device__ void operator()(const double* gx, const double* gy, const double* gz) {
     const int nb = lb + 1, nc = lc + 1, nd = ld + 1;
     long e = 0;
@@ -183,8 +183,8 @@ struct StoreConsumer {    // accumulate the Cartesian block [nca][ncb][ncc][ncd]
     for (int bx = lb; bx >= 0; --bx) for (int by = lb - bx; by >= 0; --by) { const int bz = lb - bx - by;
     for (int cx = lc; cx >= 0; --cx) for (int cy = lc - cx; cy >= 0; --cy) { const int cz = lc - cx - cy;
     for (int dx = ld; dx >= 0; --dx) for (int dy = ld - dx; dy >= 0; --dy, ++e) { const int dz = ld - dx - dy;
-      out[e] += gx[((ax * nb + bx) * nc + cx) * nd + dx] * gy[((ay * nb + by) * nc + cy) * nd + dy] *
-                gz[((az * nb + bz) * nc + cz) * nd + dz];
+      out[e * stride] += gx[((ax * nb + bx) * nc + cx) * nd + dx] * gy[((ay * nb + by) * nc + cy) * nd + dy] *
+                         gz[((az * nb + bz) * nc + cz) * nd + dz];
     }}}}
   }
 };
@@ -198,14 +198,16 @@ __global__ void __launch_bounds__(128) generic_jk_kernel(Work w) {
   quartet_loop<LC>(w, i, j, g, c);
 }
 
-// list mode only: block t of Cartesian integrals is accumulated at out + off[t] (must be zeroed by the caller)
+// list mode only: element e of block t of Cartesian integrals is accumulated at out[off[t] + e * stride] (zeroed by the caller).
+// stride 1: one contiguous block per quartet; off[t] = t, stride = number of items: element-major, so that the read-modify-write
+// of the 32 threads of a warp coalesces (the Schwarz pass of plan creation)
 template <int LC>
-__global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out, const long long* off) {
+__global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out, const long long* off, long stride) {
   int i, j; double f;
   if (!locate(w, i, j, f)) return;
   const long t = (long)(blockIdx.x * w.nshard + w.shard) * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
   QuartetGeom g; load_geom(w, i, j, g);
-  StoreConsumer c{out + off[t], g.la, g.lb, g.lc, g.ld};
+  StoreConsumer c{out + off[t], g.la, g.lb, g.lc, g.ld, stride};
   quartet_loop<LC>(w, i, j, g, c);
 }
 
@@ -313,11 +315,11 @@ cudaError_t launch_generic_jk(const Work& w, int nblocks_dense, cudaStream_t s) 
   return cudaGetLastError();
 }
 
-cudaError_t launch_generic_store(const Work& w, double* out, const long long* off, cudaStream_t s) {
+cudaError_t launch_generic_store(const Work& w, double* out, const long long* off, long stride, cudaStream_t s) {
   dim3 block(GENERIC_BJ, GENERIC_BI);
   const int grid = grid_of(w, GENERIC_BJ * GENERIC_BI, 0);
   if (grid <= 0) return cudaSuccess;
-  if (needs_hi(w)) generic_store_kernel<6><<<grid, block, 0, s>>>(w, out, off); else generic_store_kernel<4><<<grid, block, 0, s>>>(w, out, off);
+  if (needs_hi(w)) generic_store_kernel<6><<<grid, block, 0, s>>>(w, out, off, stride); else generic_store_kernel<4><<<grid, block, 0, s>>>(w, out, off, stride);
   return cudaGetLastError();
 }
 

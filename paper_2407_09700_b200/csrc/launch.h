@@ -12,7 +12,7 @@ constexpr int GENERIC_BJ = 32, GENERIC_BI = 4;
 constexpr int GENERIC_GRAD_BJ = 32, GENERIC_GRAD_BI = 4;
 
 cudaError_t launch_generic_jk(const Work& w, int nblocks_dense, cudaStream_t s);
-cudaError_t launch_generic_store(const Work& w, double* out, const long long* off, cudaStream_t s);
+cudaError_t launch_generic_store(const Work& w, double* out, const long long* off, long stride, cudaStream_t s);   // element e of item t at out[off[t] + e * stride]
 cudaError_t launch_generic_grad(const Work& w, int nblocks_dense, cudaStream_t s);
 
 // tuned kernels: a launcher per l-class; returns false in `*handled` when the class has no tuned kernel.
@@ -43,8 +43,10 @@ cudaError_t launch_cart2sph(const ShellMap& m, const double* Mcart, double* Msph
 // spherical blocks from Cartesian blocks: quartet t has shells q4[4t..4t+3], Cartesian block at cart + coff[t], output at out + ooff[t]
 cudaError_t launch_block_c2s(const ShellMap& m, const int* q4, int n, const double* cart, const long long* coff,
                              double* out, const long long* ooff, cudaStream_t s);
-// Q[t] = sqrt(max_{s,t'} |(s t'|s t')|) over spherical components from the Cartesian block (ab|ab) [nab][nab] at cart + t*nab*nab
+// Q[t] = sqrt(max_{s,t'} |(s t'|s t')|) over spherical components from the Cartesian block (ab|ab) [nab][nab], element-major:
+// element e of pair t at cart[e * n + t]
 cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, double* Q, cudaStream_t s);
+cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, cudaStream_t s);
 // density-weighted screening (transform.cu): shell-group sub-block maxima of |D|, then per unit the effective threshold,
 // the per-call kept ket counts and the number of quartets that pass
 struct DscreenUnit { const double* qb; const double* qk; const int* count; int* count_dyn; int nbra; int g[4]; };

@@ -104,7 +104,7 @@ __global__ void schwarz_diag_kernel(int la, int lb, int n, const double* __restr
   const int lane = threadIdx.x % 32;
   if (t >= n) return;
   const int nca = ncart(la), ncb = ncart(lb), nab = nca * ncb;
-  const double* M = cart + (long)t * nab * nab;
+  const double* M = cart + t;   // element-major: element e of this pair at M[e * n]
   const double* Ta = c_c2s + c2s_off(la); const double* Tb = c_c2s + c2s_off(lb);
   double best = 0.0;
   for (int st = lane; st < nsph(la) * nsph(lb); st += 32) {
@@ -113,9 +113,9 @@ __global__ void schwarz_diag_kernel(int la, int lb, int n, const double* __restr
     for (int a = 0; a < nca; ++a) { const double ta = Ta[s * nca + a]; if (ta == 0.0) continue;
       for (int b = 0; b < ncb; ++b) { const double tb = Tb[tt * ncb + b]; if (tb == 0.0) continue;
         double inner = 0.0;
-        const double* row = M + (long)(a * ncb + b) * nab;
+        const double* row = M + (long)(a * ncb + b) * nab * n;
         for (int a2 = 0; a2 < nca; ++a2) { const double ta2 = Ta[s * nca + a2]; if (ta2 == 0.0) continue;
-          for (int b2 = 0; b2 < ncb; ++b2) inner += ta2 * Tb[tt * ncb + b2] * row[a2 * ncb + b2];
+          for (int b2 = 0; b2 < ncb; ++b2) inner += ta2 * Tb[tt * ncb + b2] * row[(long)(a2 * ncb + b2) * n];
         }
         acc += ta * tb * inner;
       }
@@ -193,6 +193,12 @@ __global__ void dscreen_kernel(const DscreenUnit* __restrict__ units, const unsi
   if ((threadIdx.x & 31) == 0 && c) atomicAdd(kept + blockIdx.y, c);
 }
 
+// work list of the Schwarz pass: item t is the quartet (pair start+t | pair start+t), its Cartesian block element-major at offset t
+__global__ void diag_list_kernel(int2* __restrict__ list, long long* __restrict__ off, int start, int m) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < m) { list[t] = make_int2(start + t, start + t); off[t] = t; }
+}
+
 // 16 independent FMA chains per thread; 2 flops per FMA
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double* sink, int iters) {
   double a[16];
@@ -250,6 +256,12 @@ cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, do
     default: rys_diag_kernel<<<grid, 128, 0, s>>>(N, rys, x, n, u, w);
   }
   static_assert(RYS2_NMAX == 6, "launch_rys_diag lists the second-layout tables up to N = 6");
+  return cudaGetLastError();
+}
+
+cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, cudaStream_t s) {
+  if (m <= 0) return cudaSuccess;
+  diag_list_kernel<<<(m + 255) / 256, 256, 0, s>>>(list, off, start, m);
   return cudaGetLastError();
 }
 
