@@ -83,7 +83,7 @@ typedef struct {
   double canonical_flops;     /* per call                                                      */
   float last_ms;              /* device time of the unit's last launch; needs eri_plan_set_timing(plan,1)      */
   float last_ms_grad;
-  int32_t kernel_grad;        /* gradient kernel of the unit: 0 generic, 2 cooperative shared-memory, 3 tile */
+  int32_t kernel_grad;        /* gradient kernel of the unit: 0 generic, 2 cooperative shared-memory, 3 tile, 4 primitive-parallel */
   int32_t reserved_;
   double canonical_flops_grad;
 } eri_class_stat_t;
@@ -136,9 +136,12 @@ int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode);
  *   ERI_TUNE_TILE_FILL_SCALE  multiplies the lane-fill thresholds below which a unit is NOT given to the tile family
  *                             (default 1; 0 = tile family wherever the class is served and the HRR guard passes)
  *   ERI_TUNE_GRAD_MIN_TASKS   cooperative gradient kernel: the run of bra pairs per task (16) is halved while a unit has
- *                             fewer tasks than this (default 32768; 0 = always runs of 16) */
+ *                             fewer tasks than this (default 32768; 0 = always runs of 16)
+ *   ERI_TUNE_PGRAD_MIN_NPP    primitive quartets per shell quartet (Ka Kb Kc Kd) from which a unit of a low-l class that the tile gradient
+ *                             kernel does not take runs on the primitive-parallel gradient kernel (default 16; 1 = wherever the class is served) */
 #define ERI_TUNE_TILE_FILL_SCALE 0
 #define ERI_TUNE_GRAD_MIN_TASKS 1
+#define ERI_TUNE_PGRAD_MIN_NPP 2
 int eri_plan_set_tuning(eri_plan_t* plan, int key, double value);
 /* Multi-GPU sharding: this process evaluates only the thread blocks b with b % nranks == rank of every
  * class launch (quartets are independent units).  The outputs are then PARTIAL sums; J, K and the gradient
@@ -180,7 +183,7 @@ int eri_measure_fp64_peak(double* tflops /*HOST out*/, void* cuda_stream);
 double eri_canonical_flops(int la, int lb, int lc, int ld, int ka, int kb, int kc, int kd, int deriv);
 
 /* Test diagnostics: the tuned kernel instantiations the library holds and those this process has launched so far, as
- * newline-separated "family la lb lc ld" (family: reg, coop, tile, tgrad, cgrad; launched also: generic, generic_grad).
+ * newline-separated "family la lb lc ld" (family: reg, coop, tile, tgrad, cgrad, pgrad; launched also: generic, generic_grad).
  * Writes at most n bytes (NUL-terminated) to buf (HOST, may be NULL) and returns the size needed. */
 int eri_kernel_catalog(char* buf, int n);
 int eri_kernel_launched(char* buf, int n);

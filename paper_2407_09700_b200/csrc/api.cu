@@ -383,6 +383,7 @@ int schwarz_collect(PairClass& pc, Dev<double>& qdev) {   // after the stream ha
 // tile family only where at least TILE_MIN_FILL of the swept lanes has work and the bra chunks hold enough rows to amortise
 // the block-end reduction (measured on cfg3)
 constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3, TILE_MIN_FILL_COOP = 0.25, TILE_MIN_FILL_GRAD = 0.1;
+constexpr long long PGRAD_MIN_NPP = 16;   // half the lanes of a warp have a primitive quartet
 constexpr long long COOP_GRAD_MIN_TASKS = 32768;   // some twenty waves of 12 warps on 148 SMs: the tail of a unit is a wave of heavy tasks
 constexpr double HRR_LOSS_MAX_GRAD = 1.0e5;   // gradient tolerance is 1e-8 Ha/Bohr absolute
 constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
@@ -416,6 +417,7 @@ struct eri_plan {
   int kernel_mode = 0, timing = 0, shard = 0, nshard = 1, serial = 0;
   double tile_fill_scale = 1.0;                       // eri_plan_set_tuning: multiplies the tile family's fill thresholds
   long long grad_min_tasks = COOP_GRAD_MIN_TASKS;     // eri_plan_set_tuning: tasks per unit below which the cooperative gradient run is halved
+  long long pgrad_min_npp = PGRAD_MIN_NPP;            // eri_plan_set_tuning: primitive quartets per quartet from which the primitive-parallel gradient kernel serves a unit
   std::vector<std::unique_ptr<PairClass>> pcs;
   std::vector<std::unique_ptr<Unit>> units;
   Dev<int> sh_l, sh_sph, sh_cart, sph2sh, cart2sh;
@@ -551,6 +553,10 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
     u.kernel_grad = 2; u.gBI = ti.BI; u.gBJ = ti.BJ;
     // a warp walks its task's bra pairs one after the other: units of few, heavy quartets (the contracted core shells,
     // K^4 = 4096 primitive quartets each) get shorter runs so that they still spread over the SMs
+    // deeply contracted units of the low-l classes: the lanes of the warp own primitive quartets (pp_grad.cuh); the 2-D integrals are
+    // built on the first centres there, so the same guard as for the tile gradient kernel applies
+    if ((long long)P.npp * R.npp >= pl.pgrad_min_npp && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
+        pp_grad_info(P.la, P.lb, R.la, R.lb, &ti)) { u.kernel_grad = 4; u.gBI = ti.BI; u.gBJ = ti.BJ; }
     while (u.gBI > 1 && u.quartets / u.gBI < pl.grad_min_tasks) u.gBI /= 2;
   }
   if (!pl.is_list) {
@@ -606,7 +612,7 @@ int launch_unit(eri_plan& pl, Unit& u, bool grad, double* gJ, double* gK, cudaSt
   {
     const int k = grad ? u.kernel_grad : u.kernel;
     TunedInfo ti{};
-    const char* fam = grad ? (k == 3 ? "tgrad" : k == 2 ? "cgrad" : "generic_grad")
+    const char* fam = grad ? (k == 3 ? "tgrad" : k == 2 ? "cgrad" : k == 4 ? "pgrad" : "generic_grad")
                            : (k == 3 ? "tile" : k == 2 ? "coop" : k == 1 ? "reg" : "generic");
     (void)ti;
     log_launch(fam, w);
@@ -618,7 +624,18 @@ int launch_unit(eri_plan& pl, Unit& u, bool grad, double* gJ, double* gK, cudaSt
   } else {
     if (u.kernel_grad == 0) CK(launch_generic_grad(w, u.g_nblocks, s));
     else if (u.kernel_grad == 2) CK(launch_coop_grad_class(w, u.g_nblocks, s));
+    else if (u.kernel_grad == 4) CK(launch_pp_grad_class(w, u.g_nblocks, s));
     else CK(launch_tuned_grad(w, u.t_nblocks, s));
+  }
+  return ERI_OK;
+}
+
+int ensure_pool(eri_plan& pl) {
+  if (!pl.pool.empty()) return ERI_OK;
+  CK(cudaEventCreateWithFlags(&pl.fork_ev, cudaEventDisableTiming));
+  for (int k = 0; k < POOL_STREAMS; ++k) {
+    cudaStream_t st; CK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)); pl.pool.push_back(st);
+    cudaEvent_t e; CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); pl.pool_ev.push_back(e);
   }
   return ERI_OK;
 }
@@ -638,13 +655,7 @@ int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
     for (int k = 0; k < nu; ++k) CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
     return ERI_OK;
   }
-  if (pl.pool.empty()) {
-    CK(cudaEventCreateWithFlags(&pl.fork_ev, cudaEventDisableTiming));
-    for (int k = 0; k < POOL_STREAMS; ++k) {
-      cudaStream_t st; CK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)); pl.pool.push_back(st);
-      cudaEvent_t e; CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); pl.pool_ev.push_back(e);
-    }
-  }
+  CKI(ensure_pool(pl));
   std::vector<int>& order = grad ? pl.order_grad : pl.order;
   if ((int)order.size() != nu) {
     order.resize(nu);
@@ -688,7 +699,12 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
   // pair sets |ab, KaKb} for group(a) >= group(b) (groups sorted by (l,K), so la >= lb) -- Alg. 1 lines 3-6
   std::vector<std::unique_ptr<PairClass>> all;
   std::deque<Dev<double>> qdev;   // Schwarz factors of the classes on the device until the one synchronisation below
-  SchwarzScratch scratch;
+  // the Schwarz passes of the pair sets are independent: dealt over the plan's stream pool (each stream its own scratch), so that
+  // the sets with few, heavy pairs (the K = 8 core shells, the f shells) overlap instead of running one after the other
+  CKI(ensure_pool(pl));
+  constexpr int NSCR = 4;
+  SchwarzScratch scratch[NSCR];
+  CK(cudaStreamSynchronize(s));   // the pool streams are not ordered behind the caller's stream: everything queued there is done first
   double qmax = 0.0;
   long long pairs_total = 0;
   for (int ga = 0; ga < ng; ++ga)
@@ -703,10 +719,10 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
       pairs_total += (long long)pc->sa.size();
       CKI(upload_pair_class(b, *pc, s));
       qdev.emplace_back();
-      CKI(schwarz_enqueue(*pc, qdev.back(), scratch, s));
+      CKI(schwarz_enqueue(*pc, qdev.back(), scratch[all.size() % NSCR], pl.pool[all.size() % NSCR]));
       all.push_back(std::move(pc));
     }
-  CK(cudaStreamSynchronize(s));
+  for (int k = 0; k < NSCR; ++k) CK(cudaStreamSynchronize(pl.pool[k]));
   for (size_t k = 0; k < all.size(); ++k) {
     CKI(schwarz_collect(*all[k], qdev[k]));
     for (double q : all[k]->Q) qmax = std::max(qmax, q);
@@ -1098,6 +1114,7 @@ int eri_plan_set_tuning(eri_plan_t* plan, int key, double value) {
   CKI(ensure_init());
   if (key == ERI_TUNE_TILE_FILL_SCALE) plan->tile_fill_scale = value;
   else if (key == ERI_TUNE_GRAD_MIN_TASKS) plan->grad_min_tasks = (long long)value;
+  else if (key == ERI_TUNE_PGRAD_MIN_NPP) plan->pgrad_min_npp = (long long)value;
   else return fail(ERI_ERR_BAD_ARG, "unknown tuning key %d", key);
   return reselect_kernels(plan);
 }

@@ -27,6 +27,9 @@ cudaError_t launch_tuned_grad(const Work& w, int nblocks_dense, cudaStream_t s);
 // cooperative gradient kernel (kind 2, dense mode): info->BI x info->BJ = bra pairs per task x ket pairs per block
 bool coop_grad_info(int la, int lb, int lc, int ld, TunedInfo* info);
 cudaError_t launch_coop_grad_class(const Work& w, int nblocks_dense, cudaStream_t s);
+// primitive-parallel gradient kernel (kind 4, dense mode, pp_grad.cuh): same task shape, lanes own primitive quartets
+bool pp_grad_info(int la, int lb, int lc, int ld, TunedInfo* info);
+cudaError_t launch_pp_grad_class(const Work& w, int nblocks_dense, cudaStream_t s);
 
 void tuned_catalog(std::vector<std::string>& out);   // "family la lb lc ld" of every tuned instantiation
 

@@ -93,8 +93,8 @@ __device__ __forceinline__ void tile_grad_axis(double* __restrict__ acc, const d
 }
 
 // one differentiated axis of one root with the density products pj[e], pk[e] of the quartet read from a shared-memory column
-// (pjk[32 e], pjk[32 (NE + e)]); accumulates [J: A, B, C | K: A, B, C] of axis AX (MODE 2)
-template <int LA, int LB, int LC, int LD, int AX>
+// (pjk[STRIDE e], pjk[STRIDE (NE + e)]; STRIDE 32: a column per lane, 1: one array per warp); accumulates [J: A, B, C | K: A, B, C] of axis AX
+template <int LA, int LB, int LC, int LD, int AX, int STRIDE = 32>
 __device__ __forceinline__ void tile_grad_team_axis(double* __restrict__ acc, const double* c00, const double* c00p, const double* init,
                                                     double b10, double b01, double b00, const double* AB, const double* CD,
                                                     double ea2, double eb2, double ec2, const double* __restrict__ pjk) {
@@ -133,7 +133,7 @@ __device__ __forceinline__ void tile_grad_team_axis(double* __restrict__ acc, co
           const double dA = pa[AX] > 0 ? fma(ea2, gr[er + RA], -pa[AX] * gr[er - RA]) : ea2 * gr[er + RA];
           const double dB = pb[AX] > 0 ? fma(eb2, gr[er + RB], -pb[AX] * gr[er - RB]) : eb2 * gr[er + RB];
           const double dC = pc[AX] > 0 ? fma(ec2, gr[er + RC], -pc[AX] * gr[er - RC]) : ec2 * gr[er + RC];
-          const double tj = pjk[32 * e] * oth, tk = pjk[32 * (NE + e)] * oth;
+          const double tj = pjk[STRIDE * e] * oth, tk = pjk[STRIDE * (NE + e)] * oth;
           acc[0] = fma(dA, tj, acc[0]); acc[1] = fma(dB, tj, acc[1]); acc[2] = fma(dC, tj, acc[2]);
           acc[3] = fma(dA, tk, acc[3]); acc[4] = fma(dB, tk, acc[4]); acc[5] = fma(dC, tk, acc[5]);
           ++e;

@@ -8,6 +8,7 @@
 #include "tile_classes.h"
 #include "tile_grad_classes.h"
 #include "coop_grad_classes.h"
+#include "pp_grad_classes.h"
 
 namespace eri {
 
@@ -119,6 +120,29 @@ cudaError_t launch_coop_grad_class(const Work& w, int nblocks, cudaStream_t s) {
   return cudaErrorNotSupported;
 }
 
+// ---- primitive-parallel gradient kernel (kernel_grad 4, dense mode): task shape of the cooperative gradient kernel, PGRAD_WARPS ket pairs per block ----
+bool launch_pgrad_group0(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+bool launch_pgrad_group1(int key, const Work& w, int nblocks, cudaStream_t s, cudaError_t* err);
+static_assert(PGRAD_NGROUPS == 2, "tuned.cu lists two primitive-parallel gradient groups");
+
+bool pp_grad_info(int la, int lb, int lc, int ld, TunedInfo* info) {
+  switch (la * 1000 + lb * 100 + lc * 10 + ld) {
+#define X(a, b, c, d) case a * 1000 + b * 100 + c * 10 + d:
+    PGRAD_GROUP0(X) PGRAD_GROUP1(X)
+#undef X
+      info->kind = 4; info->TQ = 1; info->BI = 16; info->BJ = 4; return true;   // BJ = PGRAD_WARPS (pp_grad.cuh)
+    default: return false;
+  }
+}
+
+cudaError_t launch_pp_grad_class(const Work& w, int nblocks, cudaStream_t s) {
+  const int key = w.bra.la * 1000 + w.bra.lb * 100 + w.ket.la * 10 + w.ket.lb;
+  cudaError_t err = cudaErrorNotSupported;
+  if (launch_pgrad_group0(key, w, nblocks, s, &err)) return err;
+  if (launch_pgrad_group1(key, w, nblocks, s, &err)) return err;
+  return cudaErrorNotSupported;
+}
+
 bool tuned_grad_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info) {
   // (dp|ps) spills (profiles/r01d_cfg4.md: 45 GB of local-memory traffic); over long primitive loops the cooperative kernel is faster
   if (la == 2 && lb == 1 && lc == 1 && ld == 0 && npp_bra * npp_ket >= 8) return false;
@@ -161,6 +185,9 @@ void tuned_catalog(std::vector<std::string>& out) {
 #undef X
 #define X(a, b, c, d, wp, em) add("cgrad", a, b, c, d);
   CGRAD_ALL(X)
+#undef X
+#define X(a, b, c, d) add("pgrad", a, b, c, d);
+  PGRAD_GROUP0(X) PGRAD_GROUP1(X)
 #undef X
 }
 

@@ -294,7 +294,7 @@ def eri_canonical_flops(la, lb, lc, ld, ka, kb, kc, kd, deriv=False) -> float:
     return float(lib().eri_canonical_flops(la, lb, lc, ld, ka, kb, kc, kd, int(bool(deriv))))
 
 
-ERI_TUNE_TILE_FILL_SCALE, ERI_TUNE_GRAD_MIN_TASKS = 0, 1
+ERI_TUNE_TILE_FILL_SCALE, ERI_TUNE_GRAD_MIN_TASKS, ERI_TUNE_PGRAD_MIN_NPP = 0, 1, 2
 
 
 def _string_list(fn) -> list[str]:

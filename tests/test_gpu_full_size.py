@@ -173,3 +173,19 @@ def test_gradient_two_water_tz_against_oracle(eri, orc):
     gJo, gKo = orc.jk_grad(basis, D)
     assert np.abs(gJ.cpu().numpy() - gJo).max() <= GRAD_TOL
     assert np.abs(gK.cpu().numpy() - gKo).max() <= GRAD_TOL
+    # primitive-parallel gradient kernel (pp_grad.cuh) on every unit of the classes it serves, whatever the contraction depth
+    plan = eri.eri_plan_create(basis, 1e-13, want_grad=True)
+    plan.set_kernel_mode(2)
+    plan.set_tuning(eri.ERI_TUNE_PGRAD_MIN_NPP, 1)
+    kinds = {}
+    for c in plan.class_stats():
+        kinds.setdefault((c["la"], c["lb"], c["lc"], c["ld"]), set()).add(c["kernel_grad"])
+    served = {tuple(int(v) for v in x.split()[1:]) for x in eri.eri_kernel_catalog() if x.startswith("pgrad ")}
+    assert len(served) == 15 and all(kinds[c] == {4} for c in served), kinds
+    pJ, pK = plan.jk_grad(dev(D))
+    assert np.abs(pJ.cpu().numpy() - gJo).max() <= GRAD_TOL and np.abs(pK.cpu().numpy() - gKo).max() <= GRAD_TOL
+    plan.set_tuning(eri.ERI_TUNE_PGRAD_MIN_NPP, 16)             # the default rule: only the deeply contracted units
+    plan.set_kernel_mode(0)
+    assert 4 in {c["kernel_grad"] for c in plan.class_stats()}
+    qJ, qK = plan.jk_grad(dev(D))
+    assert np.abs(qJ.cpu().numpy() - gJo).max() <= GRAD_TOL and np.abs(qK.cpu().numpy() - gKo).max() <= GRAD_TOL
