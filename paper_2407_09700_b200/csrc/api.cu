@@ -434,7 +434,14 @@ struct eri_plan {
   // are dealt over a small pool of streams, heaviest first, forked from and joined to the caller's stream with events
   std::vector<cudaStream_t> pool; std::vector<cudaEvent_t> pool_ev; cudaEvent_t fork_ev = nullptr;
   std::vector<int> order, order_grad;   // unit indices by decreasing cost
+  // CUDA graph of the concurrent J/K launch schedule (the class kernels touch plan-owned buffers only): [0] plain, [1] density-weighted
+  // call.  Captured at the second call of a selection (the first one sets the kernels' attributes), replayed afterwards: one
+  // graph launch instead of some hundred kernel launches and stream/event calls -- the small workloads are launch-bound.
+  cudaGraphExec_t jk_graph[2] = {nullptr, nullptr};
+  int jk_graph_gen[2] = {-1, -1}, jk_calls[2] = {0, 0}, sel_gen = 0;
+  bool graphs_ok = true;
   ~eri_plan() {
+    for (cudaGraphExec_t g : jk_graph) if (g) cudaGraphExecDestroy(g);
     for (cudaEvent_t e : ev) cudaEventDestroy(e);
     for (cudaEvent_t e : pool_ev) cudaEventDestroy(e);
     for (cudaStream_t st : pool) cudaStreamDestroy(st);
@@ -640,22 +647,9 @@ int ensure_pool(eri_plan& pl) {
   return ERI_OK;
 }
 
-int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
+// the concurrent launch schedule: units by decreasing cost, the large ones on the caller's stream, the small ones on the pool
+int run_units_concurrent(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
   const int nu = (int)pl.units.size();
-  if (pl.timing) {   // serial, one event between launches: per-unit device times
-    while ((int)pl.ev.size() < nu + 1) { cudaEvent_t e; CK(cudaEventCreate(&e)); pl.ev.push_back(e); }
-    for (int k = 0; k < nu; ++k) {
-      CK(cudaEventRecord(pl.ev[k], s));
-      CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
-    }
-    CK(cudaEventRecord(pl.ev[nu], s)); pl.ev_pending = true; pl.ev_grad = grad;
-    return ERI_OK;
-  }
-  if (nu < 2 || pl.serial) {
-    for (int k = 0; k < nu; ++k) CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
-    return ERI_OK;
-  }
-  CKI(ensure_pool(pl));
   std::vector<int>& order = grad ? pl.order_grad : pl.order;
   if ((int)order.size() != nu) {
     order.resize(nu);
@@ -676,6 +670,46 @@ int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
   }
   for (int k = 0; k < POOL_STREAMS; ++k) { CK(cudaEventRecord(pl.pool_ev[k], pl.pool[k])); CK(cudaStreamWaitEvent(s, pl.pool_ev[k], 0)); }
   return ERI_OK;
+}
+
+int run_units(eri_plan& pl, bool grad, double* gJ, double* gK, cudaStream_t s) {
+  const int nu = (int)pl.units.size();
+  if (pl.timing) {   // serial, one event between launches: per-unit device times
+    while ((int)pl.ev.size() < nu + 1) { cudaEvent_t e; CK(cudaEventCreate(&e)); pl.ev.push_back(e); }
+    for (int k = 0; k < nu; ++k) {
+      CK(cudaEventRecord(pl.ev[k], s));
+      CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
+    }
+    CK(cudaEventRecord(pl.ev[nu], s)); pl.ev_pending = true; pl.ev_grad = grad;
+    return ERI_OK;
+  }
+  if (nu < 2 || pl.serial) {
+    for (int k = 0; k < nu; ++k) CKI(launch_unit(pl, *pl.units[k], grad, gJ, gK, s));
+    return ERI_OK;
+  }
+  CKI(ensure_pool(pl));
+  if (!grad && pl.graphs_ok) {
+    const int gi = pl.ds_active ? 1 : 0;
+    if (pl.jk_graph[gi] && pl.jk_graph_gen[gi] == pl.sel_gen) { CK(cudaGraphLaunch(pl.jk_graph[gi], s)); return ERI_OK; }
+    if (pl.jk_graph_gen[gi] != pl.sel_gen) { pl.jk_graph_gen[gi] = pl.sel_gen; pl.jk_calls[gi] = 0; if (pl.jk_graph[gi]) { cudaGraphExecDestroy(pl.jk_graph[gi]); pl.jk_graph[gi] = nullptr; } }
+    if (pl.jk_calls[gi]++ >= 1) {   // second call of this selection: capture the schedule, then replay it
+      cudaGraph_t g = nullptr;
+      if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        const int rc = run_units_concurrent(pl, false, nullptr, nullptr, s);
+        const cudaError_t ec = cudaStreamEndCapture(s, &g);
+        if (rc == ERI_OK && ec == cudaSuccess && g && cudaGraphInstantiate(&pl.jk_graph[gi], g, 0) == cudaSuccess) {
+          cudaGraphDestroy(g);
+          CK(cudaGraphLaunch(pl.jk_graph[gi], s));
+          return ERI_OK;
+        }
+        if (g) cudaGraphDestroy(g);
+        pl.jk_graph[gi] = nullptr;
+      }
+      cudaGetLastError();        // capture is an optimisation: on any failure fall back to plain launches for good
+      pl.graphs_ok = false;
+    }
+  }
+  return run_units_concurrent(pl, grad, gJ, gK, s);
 }
 
 int plan_common(eri_plan& pl, const eri_shell_t* shells, int nshell, const eri_prim_t* prims, int nprim,
@@ -990,7 +1024,7 @@ void eri_plan_destroy(eri_plan_t* plan) {
 }
 int eri_plan_set_shard(eri_plan_t* plan, int rank, int nranks) {
   if (!plan || nranks < 1 || rank < 0 || rank >= nranks) return fail(ERI_ERR_BAD_ARG, "bad shard %d of %d", rank, nranks);
-  plan->shard = rank; plan->nshard = nranks;
+  plan->shard = rank; plan->nshard = nranks; ++plan->sel_gen;
   return ERI_OK;
 }
 
@@ -1100,7 +1134,7 @@ static int reselect_kernels(eri_plan_t* plan) {
   int rc = ERI_OK;
   for (auto& u : plan->units) { rc = select_kernels(*plan, *u, st); if (rc != ERI_OK) break; }
   cudaStreamSynchronize(st); cudaStreamDestroy(st);
-  plan->order.clear(); plan->order_grad.clear();
+  plan->order.clear(); plan->order_grad.clear(); ++plan->sel_gen;
   return rc;
 }
 int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode) {

@@ -144,8 +144,6 @@ cudaError_t launch_pp_grad_class(const Work& w, int nblocks, cudaStream_t s) {
 }
 
 bool tuned_grad_info(int la, int lb, int lc, int ld, int npp_bra, int npp_ket, TunedInfo* info) {
-  // (dp|ps) spills (profiles/r01d_cfg4.md: 45 GB of local-memory traffic); over long primitive loops the cooperative kernel is faster
-  if (la == 2 && lb == 1 && lc == 1 && ld == 0 && npp_bra * npp_ket >= 8) return false;
   // few quartets with 24 primitive ket pairs (K = 3 x 8) fill the tile's 32 ket slots badly; measured on cfg4: faster on the cooperative kernel
   // for the (x|ps) classes, slower for (x|ss) and for the contracted (ds|pp), (pp|pp) units (profiles/r01f_cfg4.md)
   if (lc >= 1 && npp_ket >= 24) return false;
