@@ -93,7 +93,7 @@ __device__ __forceinline__ void fill_2d_smem(double* __restrict__ dst, int s1, i
   }
 }
 
-// Phase 1 in two stages for the eight-warp class (gg|gg).  With one lane per (root, axis) the 27 lanes that build the 2-D
+// Phase 1 in two stages for the eight-warp class (gg|gg) (and three four-warp classes, see CoopTraits::SPLIT1).  With one lane per (root, axis) the 27 lanes that build the 2-D
 // integrals work alone while the other 229 wait, and that build -- mostly the ket transfer, 25 values for each of the 25 bra
 // index pairs -- is as long as the product phase.  Stage a: lane (root, axis) runs the vertical recurrence and the bra
 // transfer and leaves B(i1, i2, m), m = 0..l3+l4, in a scratch area; stage b: the 3 N (l1+1)(l2+1) independent ket transfers
@@ -183,7 +183,9 @@ struct CoopTraits {
   static constexpr int SLAB2D = 3 * N * G2;
   static constexpr int KROW = (2 * (NC + ND)) | 1;           // per (a,b): Kac[NC] Kad[ND] Kbc[NC] Kbd[ND]; odd stride: no bank conflicts
   static constexpr int SLABK = PASSES * T * KROW;
-  static constexpr bool SPLIT1 = TW >= 8;                    // two-stage phase 1 (fill_2d_bra + ket_transfer): the slab-bound class (gg|gg)
+  // two-stage phase 1 (fill_2d_bra + ket_transfer): the slab-bound class (gg|gg) and the three four-warp classes that measured
+  // faster with it on cfg1 K = 3 ((gd|ff) 232 -> 215 ms, (gd|gd) 196 -> 186, (gg|dd) 197 -> 176; (ff|ff) 233 -> 298 and the others slower)
+  static constexpr bool SPLIT1 = TW >= 8 || (TW == 4 && LA == 4 && ((LB == 2 && LC == 3 && LD == 3) || (LB == 2 && LC == 4 && LD == 2) || (LB == 4 && LC == 2 && LD == 2)));
   static constexpr int NIJ = (LA + 1) * (LB + 1), MM1 = LC + LD + 1;
   static constexpr int SCR = SPLIT1 ? 3 * N * NIJ * MM1 : 0;    // B(i, j, m) of every (root, axis)
   static constexpr int SLAB = (SLAB2D > SLABK ? SLAB2D : SLABK) + SCR + NCD;   // + bra-transfer scratch + staged D_cd
