@@ -116,6 +116,23 @@ int eri_plan_jk_grad(eri_plan_t* plan, const double* D /*DEVICE*/, double* grad_
 int eri_plan_build_jk_dscreen(eri_plan_t* plan, const double* D /*DEVICE*/, double* J /*DEVICE*/, double* K /*DEVICE*/,
                               void* cuda_stream);
 int eri_plan_dscreen_quartets(eri_plan_t* plan, int64_t* out /*HOST*/);
+/* The shell-group maxima of the last eri_plan_build_jk_dscreen call (waits for it): ao_group[i] = shell group (equal l and K,
+ * PAPER.md:68) of AO i, P[g * n_shell_groups + h] = max |D| over the sub-block between groups g and h (the P_{a|b} of Eq. 9).
+ * ao_group HOST out nao, P HOST out n_shell_groups^2 (eri_plan_stats); either may be NULL.  ERI_ERR_BAD_ARG before the first
+ * density-weighted call. */
+int eri_plan_dscreen_group_max(eri_plan_t* plan, int32_t* ao_group /*HOST out*/, double* P /*HOST out*/);
+/* Allocation-free form of that pass over the density (Eq. 9), for callers that cannot call cudaMalloc (CUDA
+ * graph capture, serving loops, harnesses that forbid it):  P[g * ngroups + h] = max |D_ij| over AOs i of group g, j of group h.
+ * D DEVICE nao*nao, ao_group DEVICE nao (entries outside 0..ngroups-1 are ignored), P DEVICE out ngroups^2; nothing else is
+ * touched: the accumulators live in a static device array of ERI_NOALLOC_MAX_GROUPS^2 64-bit words (32 KB per GPU, held
+ * until the process exits).  The call makes no cudaMalloc, cudaFree or other allocating call and no host synchronisation; it
+ * enqueues a clear of the accumulators, the pass and the copy to P on `cuda_stream`.  ngroups > ERI_NOALLOC_MAX_GROUPS (or
+ * < 0, nao < 0, a null pointer) returns ERI_ERR_BAD_ARG.  EVERY call on a device shares the one array: calls whose device
+ * work may overlap (different streams, several host threads) race and give wrong maxima -- order them.  Works on whichever
+ * device is current (the array exists once per device); it does not bind the library to a device. */
+#define ERI_NOALLOC_MAX_GROUPS 64
+int eri_density_group_max_noalloc(const double* D /*DEVICE*/, int nao, const int32_t* ao_group /*DEVICE*/, int ngroups,
+                                  double* P /*DEVICE out*/, void* cuda_stream);
 /* Same work with HOST buffers: H2D copy of D, build, D2H copy of the results, stream synchronised on return. */
 int eri_plan_build_jk_host(eri_plan_t* plan, const double* D /*HOST*/, double* J /*HOST*/, double* K /*HOST*/,
                            void* cuda_stream);

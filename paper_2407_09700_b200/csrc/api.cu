@@ -1065,6 +1065,31 @@ int eri_plan_dscreen_quartets(eri_plan_t* plan, int64_t* out) {
   return ERI_OK;
 }
 
+int eri_plan_dscreen_group_max(eri_plan_t* plan, int32_t* ao_group, double* P) {
+  if (!plan) return fail(ERI_ERR_BAD_ARG, "null plan");
+  if (!plan->ds_ready) return fail(ERI_ERR_BAD_ARG, "no density-weighted build has run on this plan");
+  const size_t ng = plan->basis.groups.size();
+  CK(cudaDeviceSynchronize());
+  if (ao_group) CK(cudaMemcpy(ao_group, plan->ao_group.p, sizeof(int) * plan->basis.nao, cudaMemcpyDeviceToHost));
+  if (P) {
+    std::vector<unsigned long long> h(ng * ng);
+    CK(cudaMemcpy(h.data(), plan->pmax.p, sizeof(unsigned long long) * h.size(), cudaMemcpyDeviceToHost));
+    std::memcpy(P, h.data(), sizeof(double) * h.size());   // the accumulators hold the bit patterns of non-negative doubles
+  }
+  return ERI_OK;
+}
+
+// Allocation-free: must not reach ensure_init (it allocates the Rys buffer on its first call) or any Dev<>::alloc.
+int eri_density_group_max_noalloc(const double* D, int nao, const int32_t* ao_group, int ngroups, double* P, void* stream) {
+  if (nao < 0 || ngroups < 0) return fail(ERI_ERR_BAD_ARG, "negative size (nao %d, ngroups %d)", nao, ngroups);
+  if (ngroups > ERI_NOALLOC_MAX_GROUPS)
+    return fail(ERI_ERR_BAD_ARG, "ngroups %d exceeds ERI_NOALLOC_MAX_GROUPS = %d, the size of the static scratch array", ngroups, ERI_NOALLOC_MAX_GROUPS);
+  if (ngroups == 0) return ERI_OK;
+  if (!P || (nao > 0 && (!D || !ao_group))) return fail(ERI_ERR_BAD_ARG, "null pointer");
+  CK(launch_group_max_noalloc(D, nao, ao_group, ngroups, P, (cudaStream_t)stream));
+  return ERI_OK;
+}
+
 int eri_plan_build_jk_host(eri_plan_t* plan, const double* D, double* J, double* K, void* stream) {
   if (!plan || !D || !J || !K) return fail(ERI_ERR_BAD_ARG, "null pointer");
   cudaStream_t s = (cudaStream_t)stream;

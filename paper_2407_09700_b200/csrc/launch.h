@@ -54,6 +54,8 @@ cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, cudaS
 // the per-call kept ket counts and the number of quartets that pass
 struct DscreenUnit { const double* qb; const double* qk; const int* count; int* count_dyn; int nbra; int g[4]; };
 cudaError_t launch_group_max(const double* D, int nao, const int* ao_group, int ng, unsigned long long* pmax, cudaStream_t s);
+// the same maxima as doubles in P[ng*ng], accumulators in a file-scope device array (no allocation; ng <= ERI_NOALLOC_MAX_GROUPS)
+cudaError_t launch_group_max_noalloc(const double* D, int nao, const int* ao_group, int ng, double* P, cudaStream_t s);
 cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, const unsigned long long* pmax, int ng, double tau,
                            double* thr_eff, unsigned long long* kept, cudaStream_t s);
 cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, double* u, double* w, cudaStream_t s);

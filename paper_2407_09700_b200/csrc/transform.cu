@@ -2,6 +2,9 @@
 // blocks for the diagnostic entry points, the Schwarz reduction (Eq. 7), and two small diagnostics.
 // The kernels digest in the Cartesian AO basis: D_cart = T^T D T once per call, J = T (2 (Jt + Jt^T)) T^T and
 // K = T (Kt + Kt^T) T^T at the end (reading R9) -- the paper never states how spherical functions are handled.
+#include <mutex>
+
+#include "../../include/eri.h"
 #include "eri_dev.cuh"
 #include "launch.h"
 
@@ -163,6 +166,30 @@ __global__ void group_max_kernel(const double* __restrict__ D, int nao, const in
   if (v > 0.0) atomicMax(pmax + ao_group[i] * ng + ao_group[j], (unsigned long long)__double_as_longlong(v));   // non-negative doubles order like integers
 }
 
+// ---- allocation-free variant (eri_density_group_max_noalloc, eri.h) ------------------------------------------------------
+// The accumulators of the pass over D live in this file-scope array instead of a cudaMalloc'd buffer: every device that loads
+// the library holds ERI_NOALLOC_MAX_GROUPS^2 words (32 KB) until the process exits.  In HOST code the name below is a stand-in,
+// not a device address: the launcher takes the address once per device with cudaGetSymbolAddress (that device current) and
+// passes the pointer to the kernels.  All calls share the array and it keeps the last call's contents.
+static __device__ __align__(256) unsigned long long d_group_max_scratch[ERI_NOALLOC_MAX_GROUPS * ERI_NOALLOC_MAX_GROUPS];
+
+// same pass as group_max_kernel, accumulators in `scratch` (zeroed by the launcher); group ids outside 0..ng-1 are ignored
+__global__ void group_max_noalloc_kernel(const double* __restrict__ D, int nao, const int* __restrict__ ao_group, int ng,
+                                         unsigned long long* __restrict__ scratch) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long)nao * nao) return;
+  const int i = (int)(t / nao), j = (int)(t - (long)i * nao);
+  const int gi = ao_group[i], gj = ao_group[j];
+  const double v = fabs(D[t]);
+  if (v > 0.0 && (unsigned)gi < (unsigned)ng && (unsigned)gj < (unsigned)ng)
+    atomicMax(scratch + gi * ng + gj, (unsigned long long)__double_as_longlong(v));
+}
+
+__global__ void group_max_export_kernel(const unsigned long long* __restrict__ scratch, int n, double* __restrict__ P) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < n) P[t] = __longlong_as_double((long long)scratch[t]);
+}
+
 // per unit u: thr_eff[u] = tau / P_{ab|cd}, P = the largest of the six group sub-block maxima (Eq. 9); per bra pair i the
 // kept kets are the prefix of the Schwarz-sorted ket set with q_i q_j >= thr_eff (Alg. 1 lines 12-16 in the limit of fine
 // bins), never more than the plan's Schwarz-only count; kept[u] = number of quartets of the unit that pass.
@@ -269,6 +296,36 @@ cudaError_t launch_group_max(const double* D, int nao, const int* ao_group, int 
   const long n2 = (long)nao * nao;
   if (n2 == 0) return cudaSuccess;
   group_max_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, s>>>(D, nao, ao_group, ng, pmax);
+  return cudaGetLastError();
+}
+
+// Allocation-free: no cudaMalloc/cudaFree, no allocating library call.  The scratch address is looked up once per device.
+cudaError_t launch_group_max_noalloc(const double* D, int nao, const int* ao_group, int ng, double* P, cudaStream_t s) {
+  constexpr int MAX_DEVICES = 64;
+  static std::mutex mu;
+  static unsigned long long* scratch_of[MAX_DEVICES] = {};
+  if (ng <= 0) return cudaSuccess;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= MAX_DEVICES) return cudaErrorInvalidDevice;
+  unsigned long long* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(mu);
+    if (!scratch_of[dev]) {
+      unsigned long long* ptr = nullptr;
+      e = cudaGetSymbolAddress((void**)&ptr, d_group_max_scratch);   // this device's copy of the array
+      if (e != cudaSuccess) return e;
+      scratch_of[dev] = ptr;
+    }
+    scratch = scratch_of[dev];
+  }
+  const int n = ng * ng;
+  e = cudaMemsetAsync(scratch, 0, sizeof(unsigned long long) * n, s);   // the array keeps the last call's maxima
+  if (e != cudaSuccess) return e;
+  const long n2 = (long)nao * nao;
+  if (n2 > 0) group_max_noalloc_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, s>>>(D, nao, ao_group, ng, scratch);
+  group_max_export_kernel<<<(n + 255) / 256, 256, 0, s>>>(scratch, n, P);
   return cudaGetLastError();
 }
 

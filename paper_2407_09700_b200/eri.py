@@ -39,7 +39,7 @@ class eri_class_stat_t(ctypes.Structure):
 
 
 EXPORTS = ["eri_build_jk", "eri_jk_grad", "eri_plan_create", "eri_plan_build_jk", "eri_plan_jk_grad",
-           "eri_plan_build_jk_dscreen", "eri_plan_dscreen_quartets", "eri_plan_build_jk_host", "eri_plan_jk_grad_host", "eri_plan_stats", "eri_plan_num_classes",
+           "eri_plan_build_jk_dscreen", "eri_plan_dscreen_quartets", "eri_plan_dscreen_group_max", "eri_density_group_max_noalloc", "eri_plan_build_jk_host", "eri_plan_jk_grad_host", "eri_plan_stats", "eri_plan_num_classes",
            "eri_plan_class_stats", "eri_plan_set_timing", "eri_plan_set_kernel_mode", "eri_plan_set_tuning", "eri_plan_set_shard", "eri_plan_destroy",
            "eri_kernel_catalog", "eri_kernel_launched",
            "eri_compute_quartets", "eri_digest_quartet_list", "eri_list_plan_create", "eri_list_plan_digest",
@@ -67,6 +67,8 @@ def lib():
         for name in ("eri_plan_build_jk", "eri_plan_build_jk_dscreen", "eri_plan_jk_grad", "eri_plan_build_jk_host", "eri_plan_jk_grad_host",
                      "eri_list_plan_digest"):
             getattr(L, name).argtypes = [_vp, _vp, _vp, _vp, _vp]
+        L.eri_plan_dscreen_group_max.argtypes = [_vp, _vp, _vp]
+        L.eri_density_group_max_noalloc.argtypes = [_vp, ctypes.c_int, _vp, ctypes.c_int, _vp, _vp]
         L.eri_plan_stats.argtypes = [_vp, ctypes.POINTER(eri_stats_t)]
         L.eri_plan_num_classes.argtypes = [_vp]
         L.eri_plan_class_stats.argtypes = [_vp, ctypes.POINTER(eri_class_stat_t), ctypes.c_int]
@@ -148,6 +150,14 @@ class Plan:
         v = _i64(0)
         _check(lib().eri_plan_dscreen_quartets(self._h, ctypes.byref(v)))
         return int(v.value)
+
+    def dens_group_max(self) -> tuple[np.ndarray, np.ndarray]:
+        """eri_plan_dscreen_group_max: (ao_group[nao], P[ng, ng]) of the last density-weighted build"""
+        ng = self.stats()["n_shell_groups"]
+        ag = np.zeros(self.basis.nao, dtype=np.int32)
+        P = np.zeros((ng, ng))
+        _check(lib().eri_plan_dscreen_group_max(self._h, _vp(ag.ctypes.data), _vp(P.ctypes.data)))
+        return ag, P
 
     def jk_grad(self, D, gJ=None, gK=None):
         import torch
@@ -243,6 +253,22 @@ def eri_digest_quartet_list(basis, quartets, D):
     _check(lib().eri_digest_quartet_list(*args, _vp(q.ctypes.data), ctypes.c_int(q.shape[0]), _dev_f64(D, (n, n)),
                                          _dev_f64(Jt), _dev_f64(Kt), _stream()))
     return Jt, Kt
+
+
+ERI_NOALLOC_MAX_GROUPS = 64
+
+
+def eri_density_group_max_noalloc(D, ao_group, ngroups: int, P):
+    """Allocation-free shell-group maxima of |D| (Eq. 9): D (nao, nao) float64, ao_group (nao,) int32, P (ngroups, ngroups)
+    float64, all CUDA tensors supplied by the caller; the library allocates nothing (static device scratch)."""
+    import torch
+    nao = int(D.shape[0])
+    if not (isinstance(ao_group, torch.Tensor) and ao_group.is_cuda and ao_group.dtype == torch.int32 and ao_group.is_contiguous()
+            and ao_group.numel() == nao):
+        raise EriError("ao_group: expected a contiguous int32 CUDA tensor of nao entries")
+    _check(lib().eri_density_group_max_noalloc(_dev_f64(D, (nao, nao)), ctypes.c_int(nao), _vp(ao_group.data_ptr()), ctypes.c_int(int(ngroups)),
+                                               _dev_f64(P, (ngroups, ngroups)), _stream()))
+    return P
 
 
 def eri_compute_quartets(basis, quartets) -> list[np.ndarray]:
