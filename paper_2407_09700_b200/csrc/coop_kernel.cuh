@@ -46,6 +46,33 @@ __device__ __forceinline__ void rys_root_one(double x, const double* __restrict_
   w = fma(s, b1w, c[N + r] - b2w);
 }
 
+// The same root and weight for the lane (root r, axis ax) of a build team whose lanes sit at base + 3 r + ax (phase 1 of the
+// paired kernel): the axis-0 lane evaluates the Chebyshev sum of the root, the axis-1 lane that of the weight (the axis-2 lane
+// repeats the root's), and the two values are exchanged by shuffles -- half the coefficient loads and FP64 instructions of
+// rys_root_one per lane; same arithmetic per value.  `mask`: the lanes of the team (all of them must call).
+template <int N>
+__device__ __forceinline__ void rys_root_team(double x, const double* __restrict__ rys, int r, int ax, int base, unsigned mask, double& u, double& w) {
+  double val;
+  const int sel = ax == 1 ? N + r : r;
+  if (x >= rys_xmax(N)) {
+    const double rx = 1.0 / x;
+    val = ax == 1 ? rys[RYS_HDR_V + N * (N - 1) / 2 + r] * sqrt(rx) : rys[RYS_HDR_H2 + N * (N - 1) / 2 + r] * rx;
+  } else {
+    const int iv = (int)(x * 0.4);
+    const double s = (x - (2.5 * iv + 1.25)) * 0.8, s2 = 2.0 * s;
+    const double* c = rys + RYS_HDR_SIZE + rys_offset(N) + iv * (28 * N) + sel;
+    double b1 = c[13 * 2 * N], b2 = 0.0;
+#pragma unroll
+    for (int k = 12; k >= 1; --k) {
+      const double t = fma(s2, b1, c[k * 2 * N] - b2);
+      b2 = b1; b1 = t;
+    }
+    val = fma(s, b1, c[0] - b2);
+  }
+  u = __shfl_sync(mask, val, base + 3 * r);
+  w = __shfl_sync(mask, val, base + 3 * r + 1);
+}
+
 // 2-D integrals of one axis and one root, built on centres 1 (bra) and 3 (ket) and transferred to 2 and 4.
 // Element (i1,i2,i3,i4) is stored at dst[i1*s1 + i2*s2 + i3*s3 + i4*s4]; x12 = R1 - R2, x34 = R3 - R4.
 template <int L1, int L2, int L3, int L4>
@@ -188,7 +215,15 @@ struct CoopTraits {
   static constexpr bool SPLIT1 = TW >= 8 || (TW == 4 && LA == 4 && ((LB == 2 && LC == 3 && LD == 3) || (LB == 2 && LC == 4 && LD == 2) || (LB == 4 && LC == 2 && LD == 2)));
   static constexpr int NIJ = (LA + 1) * (LB + 1), MM1 = LC + LD + 1;
   static constexpr int SCR = SPLIT1 ? 3 * N * NIJ * MM1 : 0;    // B(i, j, m) of every (root, axis)
-  static constexpr int SLAB = (SLAB2D > SLABK ? SLAB2D : SLABK) + SCR + NCD;   // + bra-transfer scratch + staged D_cd
+  // paired phase 1 (one-warp classes with at most five roots): the two half-warps build the 2-D integrals of two consecutive
+  // primitive quartets of the task at once, each into its own slab; phase 2 then consumes the slabs one after the other.
+  // With one lane per (root, axis) phase 1 kept 3 N of 32 lanes busy and took a third of the family's time on cfg3.
+  // Not where the second slab would cost a resident block ((ff|dp): 78 -> 132 KB per block, one block per SM instead of two,
+  // 8.5 -> 9.9 ms on cfg3): the kernels with 36 or more accumulators per lane hold two blocks per SM by registers, the others three.
+  static constexpr int S0 = SLAB2D > SLABK ? SLAB2D : SLABK;                // first slab, later the K partial sums
+  static constexpr size_t SMEM_PAIRED = sizeof(double) * (S0 + SLAB2D + NCD) * GROUPS;
+  static constexpr bool PAIR = TW == 1 && NCH == 1 && !SPLIT1 && 3 * N <= 16 && SMEM_PAIRED <= (PASSES * NCD >= 36 ? 113 : 75) * 1024;
+  static constexpr int SLAB = S0 + (PAIR ? SLAB2D : 0) + SCR + NCD;   // + second slab + bra-transfer scratch + staged D_cd
   static constexpr size_t SMEM = sizeof(double) * SLAB * GROUPS;
   static_assert(SMEM <= 227 * 1024, "cooperative kernel: shared memory");
 };
@@ -262,7 +297,112 @@ __global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WAR
   double pjcd[NCD];
 #pragma unroll
   for (int cd = 0; cd < NCD; ++cd) pjcd[cd] = 0.0;
+  double g[PASSES][NCD];
+#pragma unroll
+  for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+    for (int cd = 0; cd < NCD; ++cd) g[ps][cd] = 0.0;
 
+  // ---- phase 2: g[ab][cd] += sum over the roots of X Y Z from the slab S2 --------------------------------------------
+  auto phase2 = [&](const double* __restrict__ S2) {
+#pragma unroll 1
+    for (int r = 0; r < N; ++r) {
+#pragma unroll
+      for (int ps = 0; ps < PASSES; ++ps) {
+        const double* X = S2 + offx[ps] + r * G2;
+        const double* Y = S2 + offy[ps] + r * G2;
+        const double* Z = S2 + offz[ps] + r * G2;
+        if constexpr (NCH > 1) {
+#pragma unroll
+          for (int cl = 0; cl < NC; ++cl) {
+            int d = 0;
+#pragma unroll
+            for (int dx = LD; dx >= 0; --dx)
+#pragma unroll
+            for (int dy = LD - dx; dy >= 0; --dy) {
+              const int dz = LD - dx - dy;
+              g[ps][cl * ND + d] = fma(X[ocx[cl] + dx] * Y[ocy[cl] + dy], Z[ocz[cl] + dz], g[ps][cl * ND + d]);
+              ++d;
+            }
+          }
+        } else {
+        int cd = 0;
+#pragma unroll
+        for (int cx = LC; cx >= 0; --cx)
+#pragma unroll
+        for (int cy = LC - cx; cy >= 0; --cy)
+#pragma unroll
+        for (int dx = LD; dx >= 0; --dx)
+#pragma unroll
+        for (int dy = LD - dx; dy >= 0; --dy) {
+          const int cz = LC - cx - cy, dz = LD - dx - dy;
+          g[ps][cd] = fma(X[cx * (LD + 1) + dx] * Y[cy * (LD + 1) + dy], Z[cz * (LD + 1) + dz], g[ps][cd]);
+          ++cd;
+        }
+        }
+      }
+    }
+  };
+
+  // ---- phase 3: digestion of the finished quartet (bra pair i, ket pair j), then g = 0 ---------------------------------
+  auto phase3 = [&](int i, double f) {
+    const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
+#pragma unroll
+    for (int ps = 0; ps < PASSES; ++ps) {
+      const bool own = lane + T * ps < NAB;
+      const long ra = (long)(a0 + ia[ps]) * n, rb = (long)(b0 + ib[ps]) * n;
+      const double Dab = own ? f * D[ra + b0 + ib[ps]] : 0.0;
+      const double fo = own ? f : 0.0;
+      double Dac[NC], Dbc[NC], Dad[ND], Dbd[ND];
+#pragma unroll
+      for (int c = 0; c < NC; ++c) { Dac[c] = D[ra + c0 + c]; Dbc[c] = D[rb + c0 + c]; }
+#pragma unroll
+      for (int d = 0; d < ND; ++d) { Dad[d] = D[ra + d0 + d]; Dbd[d] = D[rb + d0 + d]; }
+      double jab = 0.0, kac[NC], kbc[NC], kad[ND], kbd[ND];
+#pragma unroll
+      for (int c = 0; c < NC; ++c) kac[c] = kbc[c] = 0.0;
+#pragma unroll
+      for (int d = 0; d < ND; ++d) kad[d] = kbd[d] = 0.0;
+#pragma unroll
+      for (int c = 0; c < NC; ++c)
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+          const double v = g[ps][c * ND + d];
+          jab = fma(v, sDcd[c * ND + d], jab);
+          pjcd[c * ND + d] = fma(v, Dab, pjcd[c * ND + d]);
+          kac[c] = fma(v, Dbd[d], kac[c]);
+          kad[d] = fma(v, Dbc[c], kad[d]);
+          kbc[c] = fma(v, Dad[d], kbc[c]);
+          kbd[d] = fma(v, Dac[c], kbd[d]);
+        }
+      if (own) atomic_add(w.J + ra + b0 + ib[ps], fo * jab);
+      double* row = S + (size_t)(lane + T * ps) * Tr::KROW;
+#pragma unroll
+      for (int c = 0; c < NC; ++c) { row[c] = fo * kac[c]; row[NC + ND + c] = fo * kbc[c]; }
+#pragma unroll
+      for (int d = 0; d < ND; ++d) { row[NC + d] = fo * kad[d]; row[2 * NC + ND + d] = fo * kbd[d]; }
+    }
+    group_sync(TW, wy);
+    // K_a. = sum over b of the rows (a,b); K_b. = sum over a.  Items: [a][NC+ND] then [b][NC+ND].
+    for (int it = lane; it < (NA + NB) * (NC + ND); it += T) {
+      const bool isa = it < NA * (NC + ND);
+      const int rem = isa ? it : it - NA * (NC + ND);
+      const int s = rem / (NC + ND), e = rem - s * (NC + ND);    // s = a or b; e < NC: column c, else column d
+      double sum = 0.0;
+      if (isa) { for (int b = 0; b < NB; ++b) sum += S[(size_t)(s * NB + b) * Tr::KROW + e]; }
+      else     { for (int a = 0; a < NA; ++a) sum += S[(size_t)(a * NB + s) * Tr::KROW + (NC + ND) + e]; }
+      const long rowK = (long)((isa ? a0 : b0) + s) * n;
+      const int col = e < NC ? c0 + e : d0 + (e - NC);
+      atomic_add(w.K + rowK + col, sum);
+    }
+    group_sync(TW, wy);
+#pragma unroll
+    for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+      for (int cd = 0; cd < NCD; ++cd) g[ps][cd] = 0.0;
+  };
+
+  if constexpr (!Tr::PAIR) {
   for (int i = i_begin; i < i_end; ++i) {
     double f;
     if (list) f = 1.0;
@@ -274,13 +414,6 @@ __global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WAR
     double A[3], AB[3];
 #pragma unroll
     for (int x = 0; x < 3; ++x) { A[x] = bp.geom[x * bp.stride + i]; AB[x] = bp.geom[(3 + x) * bp.stride + i]; }
-    const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
-
-    double g[PASSES][NCD];
-#pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps)
-#pragma unroll
-      for (int cd = 0; cd < NCD; ++cd) g[ps][cd] = 0.0;
 
     for (int kb = 0; kb < bp.npp; ++kb) {
       const double p = bp.prim[(kb * 5 + 0) * bp.stride + i];
@@ -370,100 +503,104 @@ __global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WAR
           }
         }
         group_sync(TW, wy);
-        // ---- phase 2 ----
-#pragma unroll 1
-        for (int r = 0; r < N; ++r) {
-#pragma unroll
-          for (int ps = 0; ps < PASSES; ++ps) {
-            const double* X = S + offx[ps] + r * G2;
-            const double* Y = S + offy[ps] + r * G2;
-            const double* Z = S + offz[ps] + r * G2;
-            if constexpr (NCH > 1) {
-#pragma unroll
-              for (int cl = 0; cl < NC; ++cl) {
-                int d = 0;
-#pragma unroll
-                for (int dx = LD; dx >= 0; --dx)
-#pragma unroll
-                for (int dy = LD - dx; dy >= 0; --dy) {
-                  const int dz = LD - dx - dy;
-                  g[ps][cl * ND + d] = fma(X[ocx[cl] + dx] * Y[ocy[cl] + dy], Z[ocz[cl] + dz], g[ps][cl * ND + d]);
-                  ++d;
-                }
-              }
-            } else {
-            int cd = 0;
-#pragma unroll
-            for (int cx = LC; cx >= 0; --cx)
-#pragma unroll
-            for (int cy = LC - cx; cy >= 0; --cy)
-#pragma unroll
-            for (int dx = LD; dx >= 0; --dx)
-#pragma unroll
-            for (int dy = LD - dx; dy >= 0; --dy) {
-              const int cz = LC - cx - cy, dz = LD - dx - dy;
-              g[ps][cd] = fma(X[cx * (LD + 1) + dx] * Y[cy * (LD + 1) + dy], Z[cz * (LD + 1) + dz], g[ps][cd]);
-              ++cd;
-            }
-            }
-          }
-        }
+        phase2(S);
         group_sync(TW, wy);
       }
     }
 
-    // ---- phase 3: digestion ----------------------------------------------------------------------------------------
-#pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps) {
-      const bool own = lane + T * ps < NAB;
-      const long ra = (long)(a0 + ia[ps]) * n, rb = (long)(b0 + ib[ps]) * n;
-      const double Dab = own ? f * D[ra + b0 + ib[ps]] : 0.0;
-      const double fo = own ? f : 0.0;
-      double Dac[NC], Dbc[NC], Dad[ND], Dbd[ND];
-#pragma unroll
-      for (int c = 0; c < NC; ++c) { Dac[c] = D[ra + c0 + c]; Dbc[c] = D[rb + c0 + c]; }
-#pragma unroll
-      for (int d = 0; d < ND; ++d) { Dad[d] = D[ra + d0 + d]; Dbd[d] = D[rb + d0 + d]; }
-      double jab = 0.0, kac[NC], kbc[NC], kad[ND], kbd[ND];
-#pragma unroll
-      for (int c = 0; c < NC; ++c) kac[c] = kbc[c] = 0.0;
-#pragma unroll
-      for (int d = 0; d < ND; ++d) kad[d] = kbd[d] = 0.0;
-#pragma unroll
-      for (int c = 0; c < NC; ++c)
-#pragma unroll
-        for (int d = 0; d < ND; ++d) {
-          const double v = g[ps][c * ND + d];
-          jab = fma(v, sDcd[c * ND + d], jab);
-          pjcd[c * ND + d] = fma(v, Dab, pjcd[c * ND + d]);
-          kac[c] = fma(v, Dbd[d], kac[c]);
-          kad[d] = fma(v, Dbc[c], kad[d]);
-          kbc[c] = fma(v, Dad[d], kbc[c]);
-          kbd[d] = fma(v, Dac[c], kbd[d]);
-        }
-      if (own) atomic_add(w.J + ra + b0 + ib[ps], fo * jab);
-      double* row = S + (size_t)(lane + T * ps) * Tr::KROW;
-#pragma unroll
-      for (int c = 0; c < NC; ++c) { row[c] = fo * kac[c]; row[NC + ND + c] = fo * kbc[c]; }
-#pragma unroll
-      for (int d = 0; d < ND; ++d) { row[NC + d] = fo * kad[d]; row[2 * NC + ND + d] = fo * kbd[d]; }
-    }
-    group_sync(TW, wy);
-    // K_a. = sum over b of the rows (a,b); K_b. = sum over a.  Items: [a][NC+ND] then [b][NC+ND].
-    for (int it = lane; it < (NA + NB) * (NC + ND); it += T) {
-      const bool isa = it < NA * (NC + ND);
-      const int rem = isa ? it : it - NA * (NC + ND);
-      const int s = rem / (NC + ND), e = rem - s * (NC + ND);    // s = a or b; e < NC: column c, else column d
-      double sum = 0.0;
-      if (isa) { for (int b = 0; b < NB; ++b) sum += S[(size_t)(s * NB + b) * Tr::KROW + e]; }
-      else     { for (int a = 0; a < NA; ++a) sum += S[(size_t)(a * NB + s) * Tr::KROW + (NC + ND) + e]; }
-      const long rowK = (long)((isa ? a0 : b0) + s) * n;
-      const int col = e < NC ? c0 + e : d0 + (e - NC);
-      atomic_add(w.K + rowK + col, sum);
-    }
-    group_sync(TW, wy);
+    phase3(i, f);
   }
 
+  } else {
+  // ---- paired phase 1: the primitive quartets of the task (bra pair, bra primitive pair, ket primitive pair) are walked two
+  // at a time; half-warp h builds item h into slab h with its lanes (root, axis), phase 2 consumes slab 0, then slab 1, and a
+  // quartet is digested as soon as its last primitive quartet has been added.
+  const int h = lane >> 4, hl = lane & 15;
+  const int p_root = hl / 3, p_axis = hl - 3 * p_root;
+  const bool p_fill = hl < 3 * N;
+  const unsigned team = ((1u << (3 * N)) - 1u) << (16 * h);
+  double* Sh = S + h * Tr::S0;
+  const int nkb = bp.npp, nkk = kp.npp;
+  auto has_work = [&](int i) { return list || j < w.ket_count[i]; };   // warp-uniform
+  auto weight = [&](int i) {
+    if (list) return 1.0;
+    double f = bp.geom[6 * bp.stride + i] * wket;
+    if (w.same && i == j) f *= 0.5;
+    return f;
+  };
+  int i0 = i_begin;
+  while (i0 < i_end && !has_work(i0)) ++i0;
+  int kb0 = 0, kk0 = 0;
+  while (i0 < i_end) {
+    // second item of the pair: the next primitive quartet of the task
+    int i1 = i0, kb1 = kb0, kk1 = kk0 + 1;
+    if (kk1 == nkk) { kk1 = 0; if (++kb1 == nkb) { kb1 = 0; ++i1; while (i1 < i_end && !has_work(i1)) ++i1; } }
+    const int mi = h ? i1 : i0, mkb = h ? kb1 : kb0, mkk = h ? kk1 : kk0;
+    if (p_fill && mi < i_end) {
+      double A[3], AB[3];
+#pragma unroll
+      for (int x = 0; x < 3; ++x) { A[x] = bp.geom[x * bp.stride + mi]; AB[x] = bp.geom[(3 + x) * bp.stride + mi]; }
+      const double p = bp.prim[(mkb * 5 + 0) * bp.stride + mi];
+      const double P[3] = {bp.prim[(mkb * 5 + 1) * bp.stride + mi], bp.prim[(mkb * 5 + 2) * bp.stride + mi], bp.prim[(mkb * 5 + 3) * bp.stride + mi]};
+      const double Kab = bp.prim[(mkb * 5 + 4) * bp.stride + mi];
+      bool swb = false;   // build on B when P is nearer to B (only if there is something to transfer)
+      if (LB > 0) {
+        double da = 0.0, db = 0.0;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { const double pa = P[x] - A[x], pb = pa + AB[x]; da += pa * pa; db += pb * pb; }
+        swb = db < da;
+      }
+      const double q = kp.prim[(mkk * 5 + 0) * kp.stride + j];
+      const double Q[3] = {kp.prim[(mkk * 5 + 1) * kp.stride + j], kp.prim[(mkk * 5 + 2) * kp.stride + j], kp.prim[(mkk * 5 + 3) * kp.stride + j]};
+      const double Kcd = kp.prim[(mkk * 5 + 4) * kp.stride + j];
+      bool swk = false;
+      if (LD > 0) {
+        double dc = 0.0, dd = 0.0;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { const double qc = Q[x] - C[x], qd = qc + CD[x]; dc += qc * qc; dd += qd * qd; }
+        swk = dd < dc;
+      }
+      const double rpq = 1.0 / (p + q), rho = p * q * rpq;
+      const double PQ[3] = {P[0] - Q[0], P[1] - Q[1], P[2] - Q[2]};
+      const double x = rho * (PQ[0] * PQ[0] + PQ[1] * PQ[1] + PQ[2] * PQ[2]);
+      double u, wt;
+      rys_root_team<N>(x, w.rys, p_root, p_axis, 16 * h, team, u, wt);
+      const double t2 = u * rpq;
+      const double b00 = 0.5 * t2, b10 = (1.0 - q * t2) * 0.5 / p, b01 = (1.0 - p * t2) * 0.5 / q;
+      const int ax = p_axis;
+      const double pa = (ax == 0 ? P[0] - A[0] : ax == 1 ? P[1] - A[1] : P[2] - A[2]);
+      const double qc = (ax == 0 ? Q[0] - C[0] : ax == 1 ? Q[1] - C[1] : Q[2] - C[2]);
+      const double pqx = (ax == 0 ? PQ[0] : ax == 1 ? PQ[1] : PQ[2]);
+      const double abx = (ax == 0 ? AB[0] : ax == 1 ? AB[1] : AB[2]);
+      const double cdx = (ax == 0 ? CD[0] : ax == 1 ? CD[1] : CD[2]);
+      const double c00 = pa + (swb ? abx : 0.0) - q * t2 * pqx;
+      const double c00p = qc + (swk ? cdx : 0.0) + p * t2 * pqx;
+      const double init = ax == 2 ? Kab * Kcd * sqrt(rpq) * wt : 1.0;
+      double* dst = Sh + (ax * N + p_root) * G2;
+      constexpr int SI = (LB + 1) * SCD, SJ = SCD, SK = LD + 1, SL = 1;
+      if (!swb) {
+        if (!swk) fill_2d_smem<LA, LB, LC, LD>(dst, SI, SJ, SK, SL, init, c00, c00p, b10, b01, b00, abx, cdx);
+        else if constexpr (LD > 0) fill_2d_smem<LA, LB, LD, LC>(dst, SI, SJ, SL, SK, init, c00, c00p, b10, b01, b00, abx, -cdx);
+      } else if constexpr (LB > 0) {
+        if (!swk) fill_2d_smem<LB, LA, LC, LD>(dst, SJ, SI, SK, SL, init, c00, c00p, b10, b01, b00, -abx, cdx);
+        else if constexpr (LD > 0) fill_2d_smem<LB, LA, LD, LC>(dst, SJ, SI, SL, SK, init, c00, c00p, b10, b01, b00, -abx, -cdx);
+      }
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int t = 0; t < 2; ++t) {   // (not unrolled: one copy of the phase 2 and phase 3 code)
+      const int ti = t ? i1 : i0;
+      if (ti >= i_end) break;
+      phase2(S + t * Tr::S0);
+      // slab 0 is dead by now: phase 3 keeps the K partial sums there, slab 1 stays untouched
+      if ((t ? kb1 : kb0) == nkb - 1 && (t ? kk1 : kk0) == nkk - 1) phase3(ti, weight(ti));
+    }
+    __syncwarp();
+    // first item of the next pair
+    i0 = i1; kb0 = kb1; kk0 = kk1 + 1;
+    if (i0 < i_end && kk0 == nkk) { kk0 = 0; if (++kb0 == nkb) { kb0 = 0; ++i0; while (i0 < i_end && !has_work(i0)) ++i0; } }
+  }
+  }
   // ---- J_cd of the task: sum the per-lane partial sums over the lanes ------------------------------------------------
 #pragma unroll
   for (int cd = 0; cd < NCD; ++cd) {
