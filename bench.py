@@ -548,14 +548,14 @@ def main():
         line["density_screen"] = dens
     if args.per_class:
         with open(args.per_class, "w") as f:
-            f.write("la lb lc ld ka kb kc kd N kernel quartets ms canonical_GFLOPs TFLOP/s pct_peak unit slots\n")
+            f.write("la lb lc ld ka kb kc kd N kernel quartets ms canonical_GFLOPs TFLOP/s pct_peak unit slots tile_fill\n")
             for u, c in enumerate(classes):
                 c["unit"] = u
             for c in sorted(classes, key=lambda c: -c[key]):
                 fl = c["canonical_flops"] if kind != "grad" else c["canonical_flops_grad"]
                 tf = fl / (c[key] * 1e-3) / 1e12 if c[key] > 0 else 0.0
                 f.write(f"{c['la']} {c['lb']} {c['lc']} {c['ld']} {c['ka']} {c['kb']} {c['kc']} {c['kd']} {c['nroots']} {c['kernel_grad'] if kind == 'grad' else c['kernel']} "
-                        f"{c['quartets']} {c[key]:.4f} {fl / 1e9:.3f} {tf:.3f} {100 * tf / fp64_peak:.2f} {c['unit']} {c['slots']}\n")
+                        f"{c['quartets']} {c[key]:.4f} {fl / 1e9:.3f} {tf:.3f} {100 * tf / fp64_peak:.2f} {c['unit']} {c['slots']} {c['tile_fill_pm'] / 1000:.3f}\n")
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -84,7 +84,7 @@ typedef struct {
   float last_ms;              /* device time of the unit's last launch; needs eri_plan_set_timing(plan,1)      */
   float last_ms_grad;
   int32_t kernel_grad;        /* gradient kernel of the unit: 0 generic, 2 cooperative shared-memory, 3 tile, 4 primitive-parallel */
-  int32_t reserved_;
+  int32_t tile_fill_pm;       /* lane fill of the unit's tile decomposition in permille (quartets / swept lane slots; 0: no tiles) */
   double canonical_flops_grad;
 } eri_class_stat_t;
 
@@ -155,7 +155,7 @@ int eri_plan_set_kernel_mode(eri_plan_t* plan, int mode);
  *   ERI_TUNE_GRAD_MIN_TASKS   cooperative gradient kernel: the run of bra pairs per task (16) is halved while a unit has
  *                             fewer tasks than this (default 32768; 0 = always runs of 16)
  *   ERI_TUNE_PGRAD_MIN_NPP    primitive quartets per shell quartet (Ka Kb Kc Kd) from which a unit of a low-l class that the tile gradient
- *                             kernel does not take runs on the primitive-parallel gradient kernel (default 16; 1 = wherever the class is served) */
+ *                             kernel does not take (or fills badly) runs on the primitive-parallel gradient kernel (default 3; 1 = wherever the class is served) */
 #define ERI_TUNE_TILE_FILL_SCALE 0
 #define ERI_TUNE_GRAD_MIN_TASKS 1
 #define ERI_TUNE_PGRAD_MIN_NPP 2

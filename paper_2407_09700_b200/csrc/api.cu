@@ -383,7 +383,9 @@ int schwarz_collect(PairClass& pc, Dev<double>& qdev) {   // after the stream ha
 // tile family only where at least TILE_MIN_FILL of the swept lanes has work and the bra chunks hold enough rows to amortise
 // the block-end reduction (measured on cfg3)
 constexpr double TILE_MIN_FILL = 0.6, TILE_MIN_BRA_FILL = 0.3, TILE_MIN_FILL_COOP = 0.25, TILE_MIN_FILL_GRAD = 0.1;
-constexpr long long PGRAD_MIN_NPP = 16;   // half the lanes of a warp have a primitive quartet
+constexpr double TILE_GRAD_FILL_PP = 0.65, TILE_GRAD_FILL_PP_SHORT = 0.35;   // tile gradient kernel against the primitive-parallel one: lane fill below which the latter
+                                                                             // takes the unit, for 8 or more / fewer primitive quartets per quartet (measured on cfg4)
+constexpr long long PGRAD_MIN_NPP = 3;    // primitive quartets per quartet from which the primitive-parallel gradient kernel fills its lanes (it packs 32 / npp quartets into a warp)
 constexpr long long COOP_GRAD_MIN_TASKS = 32768;   // some twenty waves of 12 warps on 148 SMs: the tail of a unit is a wave of heavy tasks
 constexpr double HRR_LOSS_MAX_GRAD = 1.0e5;   // gradient tolerance is 1e-8 Ha/Bohr absolute
 constexpr double HRR_LOSS_MAX = 1.0e3;   // at most three digits (tile family; otherwise the cooperative family chooses the centre)
@@ -553,7 +555,15 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
     }
     // gradient: one more quantum is transferred (lb + 1, ld + 1 is not raised), so the loss bound is one power higher
     if (pl.want_grad && fill >= pl.tile_fill_scale * TILE_MIN_FILL_GRAD && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
-        tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) { u.kernel_grad = 3; u.gBI = ti.BI; }
+        tuned_grad_info(P.la, P.lb, R.la, R.lb, P.npp, R.npp, &ti)) {
+      // deeply contracted units on badly filled tiles (a contracted second ket shell has few partners per first shell: half the
+      // lanes idle, profiles/r02_cfg4.md) are left to the primitive-parallel kernel below, whose lanes own primitive quartets
+      TunedInfo tp{};
+      const long long npq = (long long)P.npp * R.npp;
+      const bool pp_better = fill < pl.tile_fill_scale * (npq >= 8 ? TILE_GRAD_FILL_PP : TILE_GRAD_FILL_PP_SHORT) && npq >= pl.pgrad_min_npp &&
+                             pp_grad_info(P.la, P.lb, R.la, R.lb, &tp);
+      if (!pp_better) { u.kernel_grad = 3; u.gBI = ti.BI; }
+    }
   }
   // cooperative gradient kernel for what the tile gradient kernel does not serve (it chooses the build centre itself)
   if (pl.kernel_mode != 1 && pl.want_grad && canonical && !pl.is_list && u.kernel_grad == 0 && coop_grad_info(P.la, P.lb, R.la, R.lb, &ti)) {
@@ -564,7 +574,10 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
     // built on the first centres there, so the same guard as for the tile gradient kernel applies
     if ((long long)P.npp * R.npp >= pl.pgrad_min_npp && P.hrr_loss_grad <= HRR_LOSS_MAX_GRAD && R.hrr_loss <= HRR_LOSS_MAX_GRAD &&
         pp_grad_info(P.la, P.lb, R.la, R.lb, &ti)) { u.kernel_grad = 4; u.gBI = ti.BI; u.gBJ = ti.BJ; }
-    while (u.gBI > 1 && u.quartets / u.gBI < pl.grad_min_tasks) u.gBI /= 2;
+    // (the primitive-parallel kernel packs 32 / npp bra pairs of a run into one warp: its runs stay at least that long)
+    const long long npq = (long long)P.npp * R.npp;
+    const int min_run = u.kernel_grad == 4 && npq < 32 ? (int)std::min<long long>(16, 32 / npq) : 1;
+    while (u.gBI > min_run && u.gBI / 2 >= min_run && u.quartets / u.gBI < pl.grad_min_tasks) u.gBI /= 2;
   }
   if (!pl.is_list) {
     std::vector<int> ro;
@@ -1146,6 +1159,7 @@ int eri_plan_class_stats(const eri_plan_t* cplan, eri_class_stat_t* out, int max
     c.slots = plan->is_list ? u.quartets : u.kernel == 3 ? u.t_slots : (long long)u.nblocks * u.BI * u.BJ;
     c.canonical_flops = u.flops; c.last_ms = u.last_ms; c.last_ms_grad = u.last_ms_grad;
     c.kernel_grad = u.kernel_grad; c.canonical_flops_grad = u.flops_grad;
+    c.tile_fill_pm = u.t_slots > 0 ? (int)(1000.0 * (double)u.quartets / (double)u.t_slots + 0.5) : 0;
   }
   return k;
 }

@@ -34,7 +34,7 @@ class eri_stats_t(ctypes.Structure):
 class eri_class_stat_t(ctypes.Structure):
     _fields_ = [("la", _i32), ("lb", _i32), ("lc", _i32), ("ld", _i32), ("ka", _i32), ("kb", _i32), ("kc", _i32),
                 ("kd", _i32), ("nroots", _i32), ("kernel", _i32), ("quartets", _i64), ("slots", _i64), ("canonical_flops", _f64),
-                ("last_ms", ctypes.c_float), ("last_ms_grad", ctypes.c_float), ("kernel_grad", _i32), ("reserved_", _i32),
+                ("last_ms", ctypes.c_float), ("last_ms_grad", ctypes.c_float), ("kernel_grad", _i32), ("tile_fill_pm", _i32),
                 ("canonical_flops_grad", _f64)]
 
 

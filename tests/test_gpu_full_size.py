@@ -184,7 +184,7 @@ def test_gradient_two_water_tz_against_oracle(eri, orc):
     assert len(served) == 15 and all(kinds[c] == {4} for c in served), kinds
     pJ, pK = plan.jk_grad(dev(D))
     assert np.abs(pJ.cpu().numpy() - gJo).max() <= GRAD_TOL and np.abs(pK.cpu().numpy() - gKo).max() <= GRAD_TOL
-    plan.set_tuning(eri.ERI_TUNE_PGRAD_MIN_NPP, 16)             # the default rule: only the deeply contracted units
+    plan.set_tuning(eri.ERI_TUNE_PGRAD_MIN_NPP, 3)              # the default rule: contracted units the tile kernel declines or fills badly
     plan.set_kernel_mode(0)
     assert 4 in {c["kernel_grad"] for c in plan.class_stats()}
     qJ, qK = plan.jk_grad(dev(D))
