@@ -560,7 +560,10 @@ int select_kernels(eri_plan& pl, Unit& u, cudaStream_t s) {
       // lanes idle, profiles/r02_cfg4.md) are left to the primitive-parallel kernel below, whose lanes own primitive quartets
       TunedInfo tp{};
       const long long npq = (long long)P.npp * R.npp;
-      const bool pp_better = fill < pl.tile_fill_scale * (npq >= 8 ? TILE_GRAD_FILL_PP : TILE_GRAD_FILL_PP_SHORT) && npq >= pl.pgrad_min_npp &&
+      // (the classes of 54 Cartesian elements run the axis-team variant of the tile kernel, three threads and two barriers per
+      // quartet: there the primitive-parallel kernel wins or ties at any fill once a quartet has three primitive quartets)
+      const int ne = ncart(P.la) * ncart(P.lb) * ncart(R.la) * ncart(R.lb);
+      const bool pp_better = (ne >= 54 || fill < pl.tile_fill_scale * (npq >= 8 ? TILE_GRAD_FILL_PP : TILE_GRAD_FILL_PP_SHORT)) && npq >= pl.pgrad_min_npp &&
                              pp_grad_info(P.la, P.lb, R.la, R.lb, &tp);
       if (!pp_better) { u.kernel_grad = 3; u.gBI = ti.BI; }
     }

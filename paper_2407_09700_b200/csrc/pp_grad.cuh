@@ -120,18 +120,32 @@ __global__ void __launch_bounds__(32 * PGRAD_WARPS) pp_grad_kernel(Work w) {
           const double c00[3] = {(P[0] - A[0]) - q * t2 * PQ[0], (P[1] - A[1]) - q * t2 * PQ[1], (P[2] - A[2]) - q * t2 * PQ[2]};
           const double c00p[3] = {(Q[0] - C[0]) + p * t2 * PQ[0], (Q[1] - C[1]) + p * t2 * PQ[1], (Q[2] - C[2]) + p * t2 * PQ[2]};
           const double init[3] = {1.0, 1.0, pref * wt[rt]};
-          double a6[6];
+          // one differentiated axis per trip of a loop that is NOT unrolled: inlined back to back, the three axis bodies share
+          // their 2 NE loads of pj, pk as common subexpressions, the compiler keeps them in registers across the bodies and spills
+          // (pp_grad_kernel<2,1,1,0>: 1.5 KB of spill stores per thread, 15.7 GB of DRAM traffic per cfg4 step, profiles/r02_cfg4.md)
+#pragma unroll 1
+          for (int axis = 0; axis < 3; ++axis) {
+            double a6[6];
 #pragma unroll
-          for (int e = 0; e < 6; ++e) a6[e] = 0.0;
-          tile_grad_team_axis<LA, LB, LC, LD, 0, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
+            for (int e = 0; e < 6; ++e) a6[e] = 0.0;
+            switch (axis) {
+              case 0:
+                tile_grad_team_axis<LA, LB, LC, LD, 0, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
 #pragma unroll
-          for (int e = 0; e < 6; ++e) { acc[(e / 3) * 9 + (e % 3) * 3 + 0] += a6[e]; a6[e] = 0.0; }
-          tile_grad_team_axis<LA, LB, LC, LD, 1, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
+                for (int e = 0; e < 6; ++e) acc[(e / 3) * 9 + (e % 3) * 3 + 0] += a6[e];
+                break;
+              case 1:
+                tile_grad_team_axis<LA, LB, LC, LD, 1, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
 #pragma unroll
-          for (int e = 0; e < 6; ++e) { acc[(e / 3) * 9 + (e % 3) * 3 + 1] += a6[e]; a6[e] = 0.0; }
-          tile_grad_team_axis<LA, LB, LC, LD, 2, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
+                for (int e = 0; e < 6; ++e) acc[(e / 3) * 9 + (e % 3) * 3 + 1] += a6[e];
+                break;
+              default:
+                tile_grad_team_axis<LA, LB, LC, LD, 2, 1>(a6, c00, c00p, init, b10, b01, b00, AB, CD, ea2, eb2, ec2, pjk);
 #pragma unroll
-          for (int e = 0; e < 6; ++e) acc[(e / 3) * 9 + (e % 3) * 3 + 2] += a6[e];
+                for (int e = 0; e < 6; ++e) acc[(e / 3) * 9 + (e % 3) * 3 + 2] += a6[e];
+                break;
+            }
+          }
         }
       }
     }
