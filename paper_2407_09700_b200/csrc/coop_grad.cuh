@@ -27,6 +27,11 @@ struct CoopGradTraits {
   static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
   static constexpr int NAB = NA * NB, NCD = NC * ND;
   static constexpr int PASSES = (NAB + 31) / 32;
+  // ab-mode with a tail: when the last pass would hold at most 8 bra component pairs ((dd|: 36 = 32 + 4, (ff|: 100 = 96 + 4),
+  // those pairs' elements are dealt over all lanes one by one (as in element mode) after the full passes
+  static constexpr int REM = NAB % 32;
+  static constexpr bool TAIL = EM == 0 && NAB > 32 && REM > 0 && REM <= 8;
+  static constexpr int PASSES_AB = TAIL ? NAB / 32 : PASSES;
   static constexpr int N = nroots_of(LA + LB + LC + LD + 1);
   static constexpr int SCD = ((LC + 2) * (LD + 1)) | 1, G2 = ((LA + 2) * (LB + 2) * SCD) | 1;   // raised on A, B, C; odd strides: no bank conflicts
   static constexpr int SLAB2D = 3 * N * G2;
@@ -136,7 +141,7 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
       }
     } else {
 #pragma unroll
-    for (int ps = 0; ps < PASSES; ++ps) {
+    for (int ps = 0; ps < Tr::PASSES_AB; ++ps) {
       int ab = lane + 32 * ps;
       const bool own = ab < NAB;
       if (!own) ab = NAB - 1;
@@ -195,6 +200,44 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
             ++d;
           }
           ++c;
+        }
+      }
+    }
+    if constexpr (Tr::TAIL) {
+      // the last NAB % 32 bra component pairs: their elements dealt over all lanes (there is no per-element accumulator, so any
+      // distribution works) instead of one more pass that keeps NAB % 32 of 32 lanes busy -- (dd|: 4 of 32
+#pragma unroll 1
+      for (int e = lane; e < Tr::REM * NCD; e += 32) {
+        const int id = e % ND, t1 = e / ND, ic = t1 % NC, ab = 32 * Tr::PASSES_AB + t1 / NC, ib = ab % NB, ia = ab / NB;
+        int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
+        cart_powers(LA, ia, ax, ay, az); cart_powers(LB, ib, bx, by, bz); cart_powers(LC, ic, cx, cy, cz); cart_powers(LD, id, dx, dy, dz);
+        const long ra = (long)(a0 + ia) * n, rb = (long)(b0 + ib) * n;
+        const double pj = D[ra + b0 + ib] * sDcd[ic * ND + id];
+        const double pk = fma(D[ra + c0 + ic], D[rb + d0 + id], D[ra + d0 + id] * D[rb + c0 + ic]);
+        const int ox = ax * SI + bx * SJ + cx * SK + dx, oy = ay * SI + by * SJ + cy * SK + dy + N * G2, oz = az * SI + bz * SJ + cz * SK + dz + 2 * N * G2;
+        // lowered terms vanish with their integer factor; the slab has no index -1, so the offset is 0 there
+        const int lax = ax > 0 ? -SI : 0, lay = ay > 0 ? -SI : 0, laz = az > 0 ? -SI : 0;
+        const int lbx = bx > 0 ? -SJ : 0, lby = by > 0 ? -SJ : 0, lbz = bz > 0 ? -SJ : 0;
+        const int lcx = cx > 0 ? -SK : 0, lcy = cy > 0 ? -SK : 0, lcz = cz > 0 ? -SK : 0;
+        const double fax = ax, fay = ay, faz = az, fbx = bx, fby = by, fbz = bz, fcx = cx, fcy = cy, fcz = cz;
+#pragma unroll 1
+        for (int rt = 0; rt < N; ++rt) {
+          const double* X = S2 + ox + rt * G2;
+          const double* Y = S2 + oy + rt * G2;
+          const double* Z = S2 + oz + rt * G2;
+          const double vx = X[0], vy = Y[0], vz = Z[0];
+          const double oyz = vy * vz, oxz = vx * vz, oxy = vx * vy;
+          const double dAx = fma(ea2, X[SI], -fax * X[lax]), dAy = fma(ea2, Y[SI], -fay * Y[lay]), dAz = fma(ea2, Z[SI], -faz * Z[laz]);
+          const double dBx = fma(eb2, X[SJ], -fbx * X[lbx]), dBy = fma(eb2, Y[SJ], -fby * Y[lby]), dBz = fma(eb2, Z[SJ], -fbz * Z[lbz]);
+          const double dCx = fma(ec2, X[SK], -fcx * X[lcx]), dCy = fma(ec2, Y[SK], -fcy * Y[lcy]), dCz = fma(ec2, Z[SK], -fcz * Z[lcz]);
+          const double jx = pj * oyz, jy = pj * oxz, jz = pj * oxy;
+          const double kx = pk * oyz, ky = pk * oxz, kz = pk * oxy;
+          acc[0] = fma(dAx, jx, acc[0]); acc[1] = fma(dAy, jy, acc[1]); acc[2] = fma(dAz, jz, acc[2]);
+          acc[3] = fma(dBx, jx, acc[3]); acc[4] = fma(dBy, jy, acc[4]); acc[5] = fma(dBz, jz, acc[5]);
+          acc[6] = fma(dCx, jx, acc[6]); acc[7] = fma(dCy, jy, acc[7]); acc[8] = fma(dCz, jz, acc[8]);
+          acc[9] = fma(dAx, kx, acc[9]); acc[10] = fma(dAy, ky, acc[10]); acc[11] = fma(dAz, kz, acc[11]);
+          acc[12] = fma(dBx, kx, acc[12]); acc[13] = fma(dBy, ky, acc[13]); acc[14] = fma(dBz, kz, acc[14]);
+          acc[15] = fma(dCx, kx, acc[15]); acc[16] = fma(dCy, ky, acc[16]); acc[17] = fma(dCz, kz, acc[17]);
         }
       }
     }
