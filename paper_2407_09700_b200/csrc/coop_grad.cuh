@@ -42,6 +42,10 @@ struct CoopGradTraits {
   // three blocks per SM by registers, the others hold two)
   static constexpr bool MINB3 = EM == 0 && WARPS == 4 && LD == 0 && LC >= 1 && LC <= 2 && NAB >= 18;   // three blocks per SM where measured faster (cfg4)
   static constexpr bool PAIR = 3 * N <= 16 && sizeof(double) * (BASE + SLAB2D + NDQ + NCD) * WARPS <= (MINB3 ? 75 : 113) * 1024;
+  // dual phase 2 (paired kernels of the classes with 18 bra component pairs, (dp|): a pass of phase 2 kept 18 of 32 lanes busy.
+  // Both slabs of a pair are consumed at once instead: half-warp h takes bra component pairs 0..15 of item h, and the two
+  // remaining pairs of each item are dealt over the 16 lanes of its half element by element.
+  static constexpr bool DUAL = PAIR && EM == 0 && NAB > 16 && NAB <= 20;
   static constexpr int SLAB = BASE + (PAIR ? SLAB2D : 0) + NDQ + NCD;               // + second slab + staged density blocks
   static constexpr size_t SMEM = sizeof(double) * SLAB * WARPS;
   static_assert(SMEM <= 227 * 1024, "slab does not fit");
@@ -103,7 +107,8 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
   };
 
   // ---- phase 2: the primitive quartet whose raised 2-D integrals are in the slab S2 adds to the 18 scalars ----------------
-  auto phase2 = [&](const double* __restrict__ S2, int i, double ea2, double eb2, double ec2) {
+  // dual = true (Tr::DUAL only): S2, i and the exponents are those of the lane's half-warp (two items at once)
+  auto phase2 = [&](const double* __restrict__ S2, int i, double ea2, double eb2, double ec2, bool dual) {
     [[maybe_unused]] const int a0 = bp.ao[i].x, b0 = bp.ao[i].y;
     if constexpr (EM != 0) {
 #pragma unroll 1
@@ -142,7 +147,7 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
     } else {
 #pragma unroll
     for (int ps = 0; ps < Tr::PASSES_AB; ++ps) {
-      int ab = lane + 32 * ps;
+      int ab = (Tr::DUAL && dual ? (lane & 15) : lane) + 32 * ps;
       const bool own = ab < NAB;
       if (!own) ab = NAB - 1;
       const int ia = ab / NB, ib = ab - ia * NB;
@@ -203,12 +208,16 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
         }
       }
     }
-    if constexpr (Tr::TAIL) {
+    if constexpr (Tr::TAIL || Tr::DUAL) {
       // the last NAB % 32 bra component pairs: their elements dealt over all lanes (there is no per-element accumulator, so any
-      // distribution works) instead of one more pass that keeps NAB % 32 of 32 lanes busy -- (dd|: 4 of 32
+      // distribution works) instead of one more pass that keeps NAB % 32 of 32 lanes busy -- (dd|: 4 of 32.  Dual phase 2: the
+      // pairs from 16 on of the half-warp's item over the 16 lanes of the half
+      const int tail_ab0 = Tr::DUAL ? 16 : 32 * Tr::PASSES_AB;
+      const int tail_n = Tr::DUAL ? (dual ? (NAB - 16) * NCD : 0) : Tr::REM * NCD;
+      const int tail_q = Tr::DUAL ? (lane & 15) : lane, tail_stride = Tr::DUAL ? 16 : 32;
 #pragma unroll 1
-      for (int e = lane; e < Tr::REM * NCD; e += 32) {
-        const int id = e % ND, t1 = e / ND, ic = t1 % NC, ab = 32 * Tr::PASSES_AB + t1 / NC, ib = ab % NB, ia = ab / NB;
+      for (int e = tail_q; e < tail_n; e += tail_stride) {
+        const int id = e % ND, t1 = e / ND, ic = t1 % NC, ab = tail_ab0 + t1 / NC, ib = ab % NB, ia = ab / NB;
         int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
         cart_powers(LA, ia, ax, ay, az); cart_powers(LB, ib, bx, by, bz); cart_powers(LC, ic, cx, cy, cz); cart_powers(LD, id, dx, dy, dz);
         const long ra = (long)(a0 + ia) * n, rb = (long)(b0 + ib) * n;
@@ -254,6 +263,23 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
     // its share of centre D = -(A + B + C) until the task ends
     warp_reduce_values<18, false>(acc, S, lane, [&](int v, int, double sum) {
       const int jk = v / 9, ce = (v % 9) / 3, ax = v % 3;
+      if (ce < 2) atomic_add((jk ? w.gK : w.gJ) + 3 * (ce == 0 ? at_ab.x : at_ab.y) + ax, sum);
+      else keepC += sum;
+      keepD -= sum;
+    });
+    __syncwarp();
+#pragma unroll
+    for (int e = 0; e < 18; ++e) acc[e] = 0.0;
+  };
+
+  // dual phase 2 with one primitive quartet per quartet: lanes 0-15 hold the sums of bra pair ia, lanes 16-31 those of ib
+  [[maybe_unused]] auto phase3_halves = [&](int ia, int ib) {
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { acc[e] *= 4.0; acc[9 + e] *= 2.0; }
+    const int2 at_a = bp.atom[ia], at_b = bp.atom[ib];
+    warp_reduce_values<18, true>(acc, S, lane, [&](int v, int half, double sum) {
+      const int jk = v / 9, ce = (v % 9) / 3, ax = v % 3;
+      const int2 at_ab = half ? at_b : at_a;
       if (ce < 2) atomic_add((jk ? w.gK : w.gJ) + 3 * (ce == 0 ? at_ab.x : at_ab.y) + ax, sum);
       else keepC += sum;
       keepD -= sum;
@@ -325,7 +351,7 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
           }
         }
         __syncwarp();
-        phase2(S, i, ea2, eb2, ec2);
+        phase2(S, i, ea2, eb2, ec2, false);
       }
     }
 
@@ -400,14 +426,25 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
       }
     }
     __syncwarp();
+    // dual phase 2: both items at once, one per half-warp, when they belong to one quartet or when every quartet is a single
+    // primitive quartet (then each half-warp holds the sums of its own quartet and phase 3 runs by halves)
+    const bool both = Tr::DUAL && i1 < i_end && (i0 == i1 || nkb * nkk == 1);
 #pragma unroll 1
     for (int t = 0; t < 2; ++t) {   // (not unrolled: one copy of the phase 2 and phase 3 code)
-      const int ti = t ? i1 : i0, tkb = t ? kb1 : kb0, tkk = t ? kk1 : kk0;
+      const int ti = both ? mi : t ? i1 : i0, tkb = both ? mkb : t ? kb1 : kb0, tkk = both ? mkk : t ? kk1 : kk0;
       if (ti >= i_end) break;
       if constexpr (EM != 0) { if (tkb == 0 && tkk == 0) stage(ti); }   // first primitive quartet of a quartet: its density blocks
       const double ea2 = 2.0 * bp.aexp[(tkb * 2 + 0) * bp.stride + ti], eb2 = 2.0 * bp.aexp[(tkb * 2 + 1) * bp.stride + ti];
       const double ec2 = 2.0 * kp.aexp[(tkk * 2 + 0) * kp.stride + j];
-      phase2(S + t * Tr::BASE, ti, ea2, eb2, ec2);
+      phase2(S + (both ? h : t) * Tr::BASE, ti, ea2, eb2, ec2, both);
+      if constexpr (Tr::DUAL) {
+        if (both) {
+          __syncwarp();   // slab 1 has been read too: the sums may be staged over both slabs
+          if (i0 != i1) phase3_halves(i0, i1);
+          else if (kb1 == nkb - 1 && kk1 == nkk - 1) phase3(i0);
+          break;
+        }
+      }
       if (tkb == nkb - 1 && tkk == nkk - 1) phase3(ti);   // slab 0 is dead by now: the lane sums are staged there
     }
     __syncwarp();
