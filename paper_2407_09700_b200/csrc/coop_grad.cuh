@@ -45,7 +45,9 @@ struct CoopGradTraits {
   // dual phase 2 (paired kernels of the classes with 18 bra component pairs, (dp|): a pass of phase 2 kept 18 of 32 lanes busy.
   // Both slabs of a pair are consumed at once instead: half-warp h takes bra component pairs 0..15 of item h, and the two
   // remaining pairs of each item are dealt over the 16 lanes of its half element by element.
-  static constexpr bool DUAL = PAIR && EM == 0 && NAB > 16 && NAB <= 20;
+  // The classes with 9 to 16 bra component pairs run the same way (no remaining pairs): two items in ab-mode on 2 NAB lanes load a
+  // sixth of what element mode loads from shared memory per element (gen_class_lists.py gives them EM = 0 where PAIR holds).
+  static constexpr bool DUAL = PAIR && EM == 0 && NAB >= 9 && NAB <= 20;
   static constexpr int SLAB = BASE + (PAIR ? SLAB2D : 0) + NDQ + NCD;               // + second slab + staged density blocks
   static constexpr size_t SMEM = sizeof(double) * SLAB * WARPS;
   static_assert(SMEM <= 227 * 1024, "slab does not fit");
