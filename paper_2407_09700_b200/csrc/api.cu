@@ -360,17 +360,23 @@ int schwarz_enqueue(PairClass& pc, Dev<double>& qdev, SchwarzScratch& sc, cudaSt
   pc.Q.assign(n, 0.0);
   if (n == 0) return ERI_OK;
   const long nab = (long)ncart(pc.la) * ncart(pc.lb), blk = nab * nab;
-  const int chunk = (int)std::max<long>(1, std::min<long>(n, (64L << 20) / blk));
-  if (sc.cart_cap < (size_t)chunk * blk) { CK(cudaStreamSynchronize(s)); sc.cart_cap = (size_t)chunk * blk; CK(sc.cart.alloc(sc.cart_cap)); }
-  if (sc.list_cap < (size_t)chunk) { CK(cudaStreamSynchronize(s)); sc.list_cap = chunk; CK(sc.list.alloc(chunk)); CK(sc.off.alloc(chunk)); }
+  // deeply contracted sets have few pairs of many primitive quartets each ((s K=8, s K=8): some hundred pairs of 4096): one thread
+  // per pair left the GPU idle for 20 ms per set (profiles/r02_plan.md); the bra primitive pairs of a pair are dealt over `split`
+  // threads instead, each with its own block, and the blocks are folded before the spherical diagonal is taken
+  const int split = pc.npp >= 16 ? std::min(pc.npp, 32) : 1;
+  const int chunk = (int)std::max<long>(1, std::min<long>(n, (64L << 20) / (blk * split)));
+  if (sc.cart_cap < (size_t)chunk * blk * split) { CK(cudaStreamSynchronize(s)); sc.cart_cap = (size_t)chunk * blk * split; CK(sc.cart.alloc(sc.cart_cap)); }
+  if (sc.list_cap < (size_t)chunk * split) { CK(cudaStreamSynchronize(s)); sc.list_cap = (size_t)chunk * split; CK(sc.list.alloc(sc.list_cap)); CK(sc.off.alloc(sc.list_cap)); }
   CK(qdev.alloc(n));
   for (int start = 0; start < n; start += chunk) {
     const int m = std::min(chunk, n - start);
-    CK(launch_diag_list(sc.list.p, sc.off.p, start, m, s));
-    CK(cudaMemsetAsync(sc.cart.p, 0, sizeof(double) * (size_t)m * blk, s));
-    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = sc.list.p; w.nlist = m; w.rys = g_rys; w.nshard = 1;
-    CK(launch_generic_store(w, sc.cart.p, sc.off.p, m, s));   // element-major blocks: coalesced accumulation
-    CK(launch_schwarz_diag(pc.la, pc.lb, m, sc.cart.p, qdev.p + start, s));
+    CK(launch_diag_list(sc.list.p, sc.off.p, start, m, split, s));
+    CK(cudaMemsetAsync(sc.cart.p, 0, sizeof(double) * (size_t)m * blk * split, s));
+    Work w{}; w.bra = pc.view(); w.ket = pc.view(); w.list = sc.list.p; w.nlist = m * split; w.rys = g_rys; w.nshard = 1;
+    w.kb_split = split; w.kb_items = m;
+    CK(launch_generic_store(w, sc.cart.p, sc.off.p, (long)m * split, s));   // element-major blocks: coalesced accumulation
+    CK(launch_fold_partials(sc.cart.p, blk, m, split, s));
+    CK(launch_schwarz_diag(pc.la, pc.lb, m, (long)m * split, sc.cart.p, qdev.p + start, s));
   }
   return ERI_OK;
 }

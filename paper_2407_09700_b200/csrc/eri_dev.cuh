@@ -176,6 +176,9 @@ struct Work {
   // density-weighted screening (Eq. 8-9; eri_plan_build_jk_dscreen): the unit's effective threshold
   // tau / P_{ab|cd} in device memory (tile family; the other families get a per-call ket_count); nullptr: use thr
   const double* thr_dev;
+  // generic store kernel, Schwarz pass of deeply contracted pair sets (api.cu schwarz_enqueue): the list holds kb_items quartets
+  // kb_split times over; copy s = t / kb_items evaluates the bra primitive pairs s, s + kb_split, ... into its own block.  0: whole quartets.
+  int kb_split, kb_items;
 };
 
 __device__ __forceinline__ void atomic_add(double* p, double v) { atomicAdd(p, v); }

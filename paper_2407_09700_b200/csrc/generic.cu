@@ -111,13 +111,13 @@ __device__ __forceinline__ void load_geom(const Work& w, int i, int j, QuartetGe
 // Loop over primitive quartets and roots; after the three 2-D integral arrays of a root are ready call
 // cons(gx, gy, gz) -- the weight and all prefactors are folded into gz.
 template <int LC, typename Consumer>
-__device__ void quartet_loop(const Work& w, int i, int j, const QuartetGeom& g, Consumer& cons) {
+__device__ void quartet_loop(const Work& w, int i, int j, const QuartetGeom& g, Consumer& cons, int kb_first = 0, int kb_step = 1) {
   const PairSet& b = w.bra; const PairSet& k = w.ket;
   const int N = nroots_of(g.la + g.lb + g.lc + g.ld);
   const int na = g.la + 1, nb = g.lb + 1, nc = g.lc + 1, nd = g.ld + 1;
   double gx[Cap<LC>::G], gy[Cap<LC>::G], gz[Cap<LC>::G];
   double u[Cap<LC>::NR], wt[Cap<LC>::NR];
-  for (int kb = 0; kb < b.npp; ++kb) {
+  for (int kb = kb_first; kb < b.npp; kb += kb_step) {
     const double p = b.prim[(kb * 5 + 0) * b.stride + i];
     const double P[3] = {b.prim[(kb * 5 + 1) * b.stride + i], b.prim[(kb * 5 + 2) * b.stride + i], b.prim[(kb * 5 + 3) * b.stride + i]};
     const double Kab = b.prim[(kb * 5 + 4) * b.stride + i];
@@ -208,7 +208,8 @@ __global__ void __launch_bounds__(128) generic_store_kernel(Work w, double* out,
   const long t = (long)(blockIdx.x * w.nshard + w.shard) * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + threadIdx.x;
   QuartetGeom g; load_geom(w, i, j, g);
   StoreConsumer c{out + off[t], g.la, g.lb, g.lc, g.ld, stride};
-  quartet_loop<LC>(w, i, j, g, c);
+  if (w.kb_split > 1) quartet_loop<LC>(w, i, j, g, c, (int)(t / w.kb_items), w.kb_split);   // a share of the bra primitive pairs
+  else quartet_loop<LC>(w, i, j, g, c);
 }
 
 // ---- gradient (Algorithm 4; Eq. 11) -------------------------------------------

@@ -48,8 +48,9 @@ cudaError_t launch_block_c2s(const ShellMap& m, const int* q4, int n, const doub
                              double* out, const long long* ooff, cudaStream_t s);
 // Q[t] = sqrt(max_{s,t'} |(s t'|s t')|) over spherical components from the Cartesian block (ab|ab) [nab][nab], element-major:
 // element e of pair t at cart[e * n + t]
-cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, double* Q, cudaStream_t s);
-cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, cudaStream_t s);
+cudaError_t launch_schwarz_diag(int la, int lb, int n, long stride, const double* cart, double* Q, cudaStream_t s);   // element e of pair t at cart[e * stride + t]
+cudaError_t launch_fold_partials(double* cart, long nelem, int m, int split, cudaStream_t s);   // sums the `split` partial blocks of the Schwarz pass into the first
+cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, int split, cudaStream_t s);
 // density-weighted screening (transform.cu): shell-group sub-block maxima of |D|, then per unit the effective threshold,
 // the per-call kept ket counts and the number of quartets that pass
 struct DscreenUnit { const double* qb; const double* qk; const int* count; int* count_dyn; int nbra; int g[4]; };

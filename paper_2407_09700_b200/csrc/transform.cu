@@ -102,12 +102,12 @@ __global__ void block_c2s_kernel(ShellMap m, const int* __restrict__ q4, const d
 }
 
 // one warp per pair: spherical diagonal (st|st) from the Cartesian block M[(ab),(a'b')]
-__global__ void schwarz_diag_kernel(int la, int lb, int n, const double* __restrict__ cart, double* __restrict__ Q) {
+__global__ void schwarz_diag_kernel(int la, int lb, int n, long stride, const double* __restrict__ cart, double* __restrict__ Q) {
   const int t = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
   const int lane = threadIdx.x % 32;
   if (t >= n) return;
   const int nca = ncart(la), ncb = ncart(lb), nab = nca * ncb;
-  const double* M = cart + t;   // element-major: element e of this pair at M[e * n]
+  const double* M = cart + t;   // element-major: element e of this pair at M[e * stride]
   const double* Ta = c_c2s + c2s_off(la); const double* Tb = c_c2s + c2s_off(lb);
   double best = 0.0;
   for (int st = lane; st < nsph(la) * nsph(lb); st += 32) {
@@ -116,9 +116,9 @@ __global__ void schwarz_diag_kernel(int la, int lb, int n, const double* __restr
     for (int a = 0; a < nca; ++a) { const double ta = Ta[s * nca + a]; if (ta == 0.0) continue;
       for (int b = 0; b < ncb; ++b) { const double tb = Tb[tt * ncb + b]; if (tb == 0.0) continue;
         double inner = 0.0;
-        const double* row = M + (long)(a * ncb + b) * nab * n;
+        const double* row = M + (long)(a * ncb + b) * nab * stride;
         for (int a2 = 0; a2 < nca; ++a2) { const double ta2 = Ta[s * nca + a2]; if (ta2 == 0.0) continue;
-          for (int b2 = 0; b2 < ncb; ++b2) inner += ta2 * Tb[tt * ncb + b2] * row[(long)(a2 * ncb + b2) * n];
+          for (int b2 = 0; b2 < ncb; ++b2) inner += ta2 * Tb[tt * ncb + b2] * row[(long)(a2 * ncb + b2) * stride];
         }
         acc += ta * tb * inner;
       }
@@ -221,9 +221,21 @@ __global__ void dscreen_kernel(const DscreenUnit* __restrict__ units, const unsi
 }
 
 // work list of the Schwarz pass: item t is the quartet (pair start+t | pair start+t), its Cartesian block element-major at offset t
-__global__ void diag_list_kernel(int2* __restrict__ list, long long* __restrict__ off, int start, int m) {
+// (split > 1: the m quartets split times over, copy s at t = s m + k; the partial blocks are folded by fold_partials_kernel)
+__global__ void diag_list_kernel(int2* __restrict__ list, long long* __restrict__ off, int start, int m, int split) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t < m) { list[t] = make_int2(start + t, start + t); off[t] = t; }
+  if (t < m * split) { const int k = t % m; list[t] = make_int2(start + k, start + k); off[t] = t; }
+}
+
+// cart[e * m * split + k] += the same element of the copies s = 1 .. split - 1 (at + s m)
+__global__ void fold_partials_kernel(double* __restrict__ cart, long nelem, int m, int split) {
+  const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nelem * m) return;
+  const long e = idx / m; const int k = (int)(idx - e * m);
+  double* p = cart + e * (long)m * split + k;
+  double sum = p[0];
+  for (int s = 1; s < split; ++s) sum += p[(long)s * m];
+  p[0] = sum;
 }
 
 // 16 independent FMA chains per thread; 2 flops per FMA
@@ -267,9 +279,16 @@ cudaError_t launch_block_c2s(const ShellMap& m, const int* q4, int n, const doub
   return cudaGetLastError();
 }
 
-cudaError_t launch_schwarz_diag(int la, int lb, int n, const double* cart, double* Q, cudaStream_t s) {
+cudaError_t launch_schwarz_diag(int la, int lb, int n, long stride, const double* cart, double* Q, cudaStream_t s) {
   if (n <= 0) return cudaSuccess;
-  schwarz_diag_kernel<<<(n + 3) / 4, 128, 0, s>>>(la, lb, n, cart, Q);
+  schwarz_diag_kernel<<<(n + 3) / 4, 128, 0, s>>>(la, lb, n, stride, cart, Q);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fold_partials(double* cart, long nelem, int m, int split, cudaStream_t s) {
+  if (split <= 1 || m <= 0) return cudaSuccess;
+  const long tot = nelem * m;
+  fold_partials_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(cart, nelem, m, split);
   return cudaGetLastError();
 }
 
@@ -286,9 +305,9 @@ cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, do
   return cudaGetLastError();
 }
 
-cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, cudaStream_t s) {
+cudaError_t launch_diag_list(int2* list, long long* off, int start, int m, int split, cudaStream_t s) {
   if (m <= 0) return cudaSuccess;
-  diag_list_kernel<<<(m + 255) / 256, 256, 0, s>>>(list, off, start, m);
+  diag_list_kernel<<<(m * split + 255) / 256, 256, 0, s>>>(list, off, start, m, split);
   return cudaGetLastError();
 }
 
