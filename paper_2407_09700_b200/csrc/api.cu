@@ -245,6 +245,7 @@ struct PairClass {
   // tile family: the same pairs in chunks of 32 slots that share the first shell (padding slots have Q = -1);
   // chunks are ordered by decreasing largest Schwarz factor, which is the factor of the chunk's first slot
   std::unique_ptr<PairClass> grouped;
+  std::vector<int> src;            // grouped only: index of every slot's pair in the Schwarz-sorted set (padding slots repeat a pair of their half)
   std::vector<double> half_q;      // grouped only: largest Schwarz factor of each half-chunk of 16 slots (sorted by it, descending; -1: padding)
   double fill = 0.0;               // grouped only: valid slots / slots
   double hrr_loss_grad = 1.0;      // the same with lb + 1 quanta (gradient kernels raise the second shell too)
@@ -293,20 +294,47 @@ int upload_pair_class(const Basis& b, PairClass& pc, cudaStream_t s) {
   return ERI_OK;
 }
 
+// The records of dst's pairs (dst.sa/sb/wgt/Q filled; pair i of dst is pair idx[i] of src) gathered on the device from src's
+// arrays -- bit-identical to upload_pair_class, without rebuilding them on the host and sending them over PCIe a second time.
+// Runs on the allocator's private stream and is complete on return, like Dev::upload.
+int gather_pair_class(const PairClass& src, const std::vector<int>& idx, PairClass& dst) {
+  const int n = dst.npair = (int)idx.size();
+  dst.stride = (n + 31) / 32 * 32;
+  if (n == 0) return ERI_OK;
+  const size_t st = dst.stride;
+  CK(dst.prim.alloc((size_t)dst.npp * 5 * st)); CK(dst.geom.alloc(7 * st)); CK(dst.aexp.alloc((size_t)dst.npp * 2 * st));
+  CK(dst.ao.alloc(st)); CK(dst.atom.alloc(st));
+  Dev<int> idxd;
+  CK(idxd.upload(idx, g_alloc_stream));
+  std::vector<double> q(st, 0.0);
+  for (int i = 0; i < n; ++i) q[i] = dst.Q[i];
+  CK(dst.q.upload(q, g_alloc_stream));
+  cudaStream_t as = g_alloc_stream;
+  CK(cudaMemsetAsync(dst.prim.p, 0, sizeof(double) * dst.prim.n, as)); CK(cudaMemsetAsync(dst.geom.p, 0, sizeof(double) * dst.geom.n, as));
+  CK(cudaMemsetAsync(dst.aexp.p, 0, sizeof(double) * dst.aexp.n, as));
+  CK(cudaMemsetAsync(dst.ao.p, 0, sizeof(int2) * st, as)); CK(cudaMemsetAsync(dst.atom.p, 0, sizeof(int2) * st, as));
+  CK(launch_gather_rows(src.prim.p, dst.prim.p, idxd.p, n, dst.npp * 5, src.stride, st, as));
+  CK(launch_gather_rows(src.geom.p, dst.geom.p, idxd.p, n, 7, src.stride, st, as));
+  CK(launch_gather_rows(src.aexp.p, dst.aexp.p, idxd.p, n, dst.npp * 2, src.stride, st, as));
+  CK(launch_gather_int2(src.ao.p, dst.ao.p, idxd.p, n, as)); CK(launch_gather_int2(src.atom.p, dst.atom.p, idxd.p, n, as));
+  CK(cudaStreamSynchronize(as));   // idxd is released on return
+  return ERI_OK;
+}
+
 // digits lost by the horizontal transfer when the 2-D integrals are built on the FIRST centre: |AB| / |PB| = p / alpha_a per quantum
 double hrr_loss_of(const Basis& b, const PairClass& pc, int extra) {
   if (pc.lb + extra == 0) return 1.0;
-  double worst = 1.0;
+  double ratio = 1.0;   // the power is monotonic: the largest p / alpha_a decides (one pow instead of one per primitive pair)
   for (size_t i = 0; i < pc.sa.size(); ++i) {
     const eri_shell_t& A = b.sh[pc.sa[i]]; const eri_shell_t& B = b.sh[pc.sb[i]];
     if (A.atom == B.atom) continue;   // AB = 0: the transfer adds nothing
     for (int ka = 0; ka < A.nprim; ++ka)
       for (int kb = 0; kb < B.nprim; ++kb) {
         const double ea = b.pr[A.prim_off + ka].exp, eb = b.pr[B.prim_off + kb].exp;
-        worst = std::max(worst, std::pow((ea + eb) / ea, pc.lb + extra));
+        ratio = std::max(ratio, (ea + eb) / ea);
       }
   }
-  return worst;
+  return std::pow(ratio, pc.lb + extra);
 }
 
 void init_pair_class(const Basis& b, int ga, int gb, PairClass& pc);
@@ -332,12 +360,12 @@ int make_grouped(const Basis& b, PairClass& pc, cudaStream_t s) {
     gp->half_q.push_back(c.q);
     for (int t = 0; t < HALF; ++t) {
       const int src = (*c.idx)[c.begin + (t < c.n ? t : 0)];   // padding repeats a pair of the half (valid addresses, same first shell)
-      gp->sa.push_back(pc.sa[src]); gp->sb.push_back(pc.sb[src]); gp->wgt.push_back(pc.wgt[src]);
+      gp->sa.push_back(pc.sa[src]); gp->sb.push_back(pc.sb[src]); gp->wgt.push_back(pc.wgt[src]); gp->src.push_back(src);
       gp->Q.push_back(t < c.n ? pc.Q[src] : -1.0);
     }
   }
   gp->fill = nvalid == 0 ? 0.0 : (double)pc.npair / ((double)HALF * nvalid);
-  CKI(upload_pair_class(b, *gp, s));
+  CKI(gather_pair_class(pc, gp->src, *gp));
   pc.grouped = std::move(gp);
   return ERI_OK;
 }
@@ -795,7 +823,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
     auto np = std::make_unique<PairClass>();
     init_pair_class(b, pc->ga, pc->gb, *np);
     for (int i : idx) { np->sa.push_back(pc->sa[i]); np->sb.push_back(pc->sb[i]); np->wgt.push_back(pc->wgt[i]); np->Q.push_back(pc->Q[i]); }
-    CKI(upload_pair_class(b, *np, s));
+    CKI(gather_pair_class(*pc, idx, *np));
     np->hrr_loss = hrr_loss_of(b, *np, 0); np->hrr_loss_grad = hrr_loss_of(b, *np, 1);
     CKI(make_grouped(b, *np, s));
     pairs_kept += np->npair;

@@ -59,6 +59,9 @@ cudaError_t launch_group_max(const double* D, int nao, const int* ao_group, int 
 cudaError_t launch_group_max_noalloc(const double* D, int nao, const int* ao_group, int ng, double* P, cudaStream_t s);
 cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, const unsigned long long* pmax, int ng, double tau,
                            double* thr_eff, unsigned long long* kept, cudaStream_t s);
+// dst[r * dstride + i] = src[r * sstride + idx[i]], r < rows, i < n (SoA pair records); dst[i] = src[idx[i]] for the int2 arrays
+cudaError_t launch_gather_rows(const double* src, double* dst, const int* idx, int n, int rows, long sstride, long dstride, cudaStream_t s);
+cudaError_t launch_gather_int2(const int2* src, int2* dst, const int* idx, int n, cudaStream_t s);
 cudaError_t launch_rys_diag(int N, const double* rys, const double* x, int n, double* u, double* w, cudaStream_t s);
 cudaError_t launch_fp64_peak(double* sink, int iters, int blocks, cudaStream_t s);
 

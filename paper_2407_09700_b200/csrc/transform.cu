@@ -238,6 +238,20 @@ __global__ void fold_partials_kernel(double* __restrict__ cart, long nelem, int 
   p[0] = sum;
 }
 
+// pair records of a reordered subset of a pair set (plan creation: the Schwarz-sorted kept set and its grouped twin are
+// gathered on the device from the set that the Schwarz pass used, instead of being rebuilt on the host and uploaded again)
+__global__ void gather_rows_kernel(const double* __restrict__ src, double* __restrict__ dst, const int* __restrict__ idx, int n, int rows,
+                                   long sstride, long dstride) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long)rows * n) return;
+  const int r = (int)(t / n), i = (int)(t - (long)r * n);
+  dst[r * dstride + i] = src[r * sstride + idx[i]];
+}
+__global__ void gather_int2_kernel(const int2* __restrict__ src, int2* __restrict__ dst, const int* __restrict__ idx, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = src[idx[i]];
+}
+
 // 16 independent FMA chains per thread; 2 flops per FMA
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double* sink, int iters) {
   double a[16];
@@ -352,6 +366,19 @@ cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, c
                            double* thr_eff, unsigned long long* kept, cudaStream_t s) {
   if (nunits == 0) return cudaSuccess;
   dscreen_kernel<<<dim3((max_nbra + 127) / 128, nunits), 128, 0, s>>>(units, pmax, ng, tau, thr_eff, kept);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_gather_rows(const double* src, double* dst, const int* idx, int n, int rows, long sstride, long dstride, cudaStream_t s) {
+  const long tot = (long)rows * n;
+  if (tot <= 0) return cudaSuccess;
+  gather_rows_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(src, dst, idx, n, rows, sstride, dstride);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_gather_int2(const int2* src, int2* dst, const int* idx, int n, cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  gather_int2_kernel<<<(n + 255) / 256, 256, 0, s>>>(src, dst, idx, n);
   return cudaGetLastError();
 }
 
