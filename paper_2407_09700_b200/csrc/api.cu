@@ -321,6 +321,33 @@ int gather_pair_class(const PairClass& src, const std::vector<int>& idx, PairCla
   return ERI_OK;
 }
 
+// The basis on the device, for building pair records there (dense plans: 9e5 primitive pairs at cfg3 took the host 40 ms to
+// build and send; profiles/r02_plan.md)
+struct BasisDev { Dev<eri_shell_t> sh; Dev<eri_prim_t> pr; Dev<double> xyz; Dev<int> cart_off; };
+int upload_basis(const Basis& b, BasisDev& d, cudaStream_t s) {
+  CK(d.sh.upload(b.sh, s)); CK(d.pr.upload(b.pr, s)); CK(d.xyz.upload(b.xyz, s)); CK(d.cart_off.upload(b.cart_off, s));
+  return ERI_OK;
+}
+// as upload_pair_class, the records computed on the device (pc.wgt is the rule 1/2 for a shell with itself, as everywhere)
+int build_pair_class_device(const BasisDev& bd, PairClass& pc) {
+  const int n = pc.npair = (int)pc.sa.size();
+  pc.stride = (n + 31) / 32 * 32;
+  if (n == 0) return ERI_OK;
+  const size_t st = pc.stride;
+  CK(pc.prim.alloc((size_t)pc.npp * 5 * st)); CK(pc.geom.alloc(7 * st)); CK(pc.aexp.alloc((size_t)pc.npp * 2 * st)); CK(pc.q.alloc(st));
+  CK(pc.ao.alloc(st)); CK(pc.atom.alloc(st));
+  Dev<int> sad, sbd;
+  CK(sad.upload(pc.sa, g_alloc_stream)); CK(sbd.upload(pc.sb, g_alloc_stream));
+  cudaStream_t as = g_alloc_stream;
+  CK(cudaMemsetAsync(pc.prim.p, 0, sizeof(double) * pc.prim.n, as)); CK(cudaMemsetAsync(pc.geom.p, 0, sizeof(double) * pc.geom.n, as));
+  CK(cudaMemsetAsync(pc.aexp.p, 0, sizeof(double) * pc.aexp.n, as)); CK(cudaMemsetAsync(pc.q.p, 0, sizeof(double) * st, as));
+  CK(cudaMemsetAsync(pc.ao.p, 0, sizeof(int2) * st, as)); CK(cudaMemsetAsync(pc.atom.p, 0, sizeof(int2) * st, as));
+  CK(launch_build_pairs(bd.sh.p, bd.pr.p, bd.xyz.p, bd.cart_off.p, sad.p, sbd.p, n, pc.Kb, pc.npp, (long)st, std::sqrt(2.0) * std::pow(PI, 1.25), pc.prim.p, pc.geom.p, pc.aexp.p,
+                        pc.ao.p, pc.atom.p, as));
+  CK(cudaStreamSynchronize(as));   // sad, sbd are released on return; the records can be used on any stream
+  return ERI_OK;
+}
+
 // digits lost by the horizontal transfer when the 2-D integrals are built on the FIRST centre: |AB| / |PB| = p / alpha_a per quantum
 double hrr_loss_of(const Basis& b, const PairClass& pc, int extra) {
   if (pc.lb + extra == 0) return 1.0;
@@ -788,6 +815,8 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
   CKI(ensure_pool(pl));
   constexpr int NSCR = 4;
   SchwarzScratch scratch[NSCR];
+  BasisDev bdev;
+  CKI(upload_basis(b, bdev, s));
   CK(cudaStreamSynchronize(s));   // the pool streams are not ordered behind the caller's stream: everything queued there is done first
   double qmax = 0.0;
   long long pairs_total = 0;
@@ -801,7 +830,7 @@ int create_dense_plan(const eri_shell_t* shells, int nshell, const eri_prim_t* p
           pc->sa.push_back(A[ia]); pc->sb.push_back(B[ib]); pc->wgt.push_back(A[ia] == B[ib] ? 0.5 : 1.0);
         }
       pairs_total += (long long)pc->sa.size();
-      CKI(upload_pair_class(b, *pc, s));
+      CKI(build_pair_class_device(bdev, *pc));
       qdev.emplace_back();
       CKI(schwarz_enqueue(*pc, qdev.back(), scratch[all.size() % NSCR], pl.pool[all.size() % NSCR]));
       all.push_back(std::move(pc));

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <string>
 #include <vector>
+#include "../../include/eri.h"
 #include "eri_dev.cuh"
 
 namespace eri {
@@ -59,6 +60,9 @@ cudaError_t launch_group_max(const double* D, int nao, const int* ao_group, int 
 cudaError_t launch_group_max_noalloc(const double* D, int nao, const int* ao_group, int ng, double* P, cudaStream_t s);
 cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, const unsigned long long* pmax, int ng, double tau,
                            double* thr_eff, unsigned long long* kept, cudaStream_t s);
+// primitive-pair records of the pairs (sa[i], sb[i]) from the shell data on the device (plan creation); arrays zeroed by the caller
+cudaError_t launch_build_pairs(const eri_shell_t* sh, const eri_prim_t* pr, const double* xyz, const int* cart_off, const int* sa, const int* sb,
+                               int n, int Kb, int npp, long st, double kfac /* sqrt(2) pi^(5/4) */, double* prim, double* geom, double* aexp, int2* ao, int2* atom, cudaStream_t s);
 // dst[r * dstride + i] = src[r * sstride + idx[i]], r < rows, i < n (SoA pair records); dst[i] = src[idx[i]] for the int2 arrays
 cudaError_t launch_gather_rows(const double* src, double* dst, const int* idx, int n, int rows, long sstride, long dstride, cudaStream_t s);
 cudaError_t launch_gather_int2(const int2* src, int2* dst, const int* idx, int n, cudaStream_t s);

@@ -238,6 +238,38 @@ __global__ void fold_partials_kernel(double* __restrict__ cart, long nelem, int 
   p[0] = sum;
 }
 
+// Primitive-pair records of a pair set (eri_dev.cuh "Pair set") computed on the device from the shell data: thread (pair i,
+// primitive pair k) writes p, P, K_ab and the two exponents; k = 0 also writes the pair's geometry, AO offsets and atoms.
+// Same formulas as upload_pair_class (api.cu), which serves the list plans from the host.
+__global__ void build_pairs_kernel(const eri_shell_t* __restrict__ sh, const eri_prim_t* __restrict__ pr, const double* __restrict__ xyz,
+                                   const int* __restrict__ cart_off, const int* __restrict__ sa, const int* __restrict__ sb, int n, int Kb, int npp,
+                                   long st, double kfac, double* __restrict__ prim, double* __restrict__ geom, double* __restrict__ aexp,
+                                   int2* __restrict__ ao, int2* __restrict__ atom) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long)n * npp) return;
+  const int k = (int)(t / n), i = (int)(t - (long)k * n);
+  const eri_shell_t A = sh[sa[i]], B = sh[sb[i]];
+  const double RA[3] = {xyz[3 * A.atom], xyz[3 * A.atom + 1], xyz[3 * A.atom + 2]};
+  const double RB[3] = {xyz[3 * B.atom], xyz[3 * B.atom + 1], xyz[3 * B.atom + 2]};
+  const double ab[3] = {RA[0] - RB[0], RA[1] - RB[1], RA[2] - RB[2]};
+  const double r2 = ab[0] * ab[0] + ab[1] * ab[1] + ab[2] * ab[2];
+  const int ka = k / Kb, kb = k - ka * Kb;
+  const eri_prim_t pa = pr[A.prim_off + ka], pb = pr[B.prim_off + kb];
+  const double p = pa.exp + pb.exp;
+  prim[((long)k * 5 + 0) * st + i] = p;
+#pragma unroll
+  for (int x = 0; x < 3; ++x) prim[((long)k * 5 + 1 + x) * st + i] = (pa.exp * RA[x] + pb.exp * RB[x]) / p;
+  prim[((long)k * 5 + 4) * st + i] = kfac / p * pa.coef * pb.coef * exp(-pa.exp * pb.exp / p * r2);
+  aexp[((long)k * 2 + 0) * st + i] = pa.exp; aexp[((long)k * 2 + 1) * st + i] = pb.exp;
+  if (k == 0) {
+#pragma unroll
+    for (int x = 0; x < 3; ++x) { geom[x * st + i] = RA[x]; geom[(3 + x) * st + i] = ab[x]; }
+    geom[6 * st + i] = sa[i] == sb[i] ? 0.5 : 1.0;
+    ao[i] = make_int2(cart_off[sa[i]], cart_off[sb[i]]);
+    atom[i] = make_int2(A.atom, B.atom);
+  }
+}
+
 // pair records of a reordered subset of a pair set (plan creation: the Schwarz-sorted kept set and its grouped twin are
 // gathered on the device from the set that the Schwarz pass used, instead of being rebuilt on the host and uploaded again)
 __global__ void gather_rows_kernel(const double* __restrict__ src, double* __restrict__ dst, const int* __restrict__ idx, int n, int rows,
@@ -366,6 +398,14 @@ cudaError_t launch_dscreen(const DscreenUnit* units, int nunits, int max_nbra, c
                            double* thr_eff, unsigned long long* kept, cudaStream_t s) {
   if (nunits == 0) return cudaSuccess;
   dscreen_kernel<<<dim3((max_nbra + 127) / 128, nunits), 128, 0, s>>>(units, pmax, ng, tau, thr_eff, kept);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_build_pairs(const eri_shell_t* sh, const eri_prim_t* pr, const double* xyz, const int* cart_off, const int* sa, const int* sb,
+                               int n, int Kb, int npp, long st, double kfac, double* prim, double* geom, double* aexp, int2* ao, int2* atom, cudaStream_t s) {
+  const long tot = (long)n * npp;
+  if (tot <= 0) return cudaSuccess;
+  build_pairs_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(sh, pr, xyz, cart_off, sa, sb, n, Kb, npp, st, kfac, prim, geom, aexp, ao, atom);
   return cudaGetLastError();
 }
 
