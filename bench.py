@@ -8,7 +8,8 @@ One "step" = one pass of the whole hot path (Rys roots, re
 digestion, final symmetrisation) over the whole kept quartet list of the workload, i.e. one eri_plan_build_jk call
 (cfg4: one eri_plan_jk_grad call; cfg1: one eri_list_plan_digest call).  The plan (S0: pair data, Schwarz bounds,
 task lists) depends on geometry, basis and threshold only, is built once before the timed region and its host time
-is reported as plan_ms; the one-shot eri_build_jk (plan + build) is timed once and reported as oneshot_ms.
+is reported as plan_ms (plan_ms_second_plan: the same input planned again, without the one-time code loading of a
+process's first plan); the one-shot eri_build_jk (plan + build) is timed once and reported as oneshot_ms.
 Default workload: cfg3, the 32-water / 1856-function J/K build the metric is quoted on.
 
 Prints ONE JSON line (rank 0).  value = unique shell quartets evaluated per second over all ranks (the metric's
@@ -485,7 +486,7 @@ def main():
         else:
             plan.build_jk_host(Dp.numpy(), Jp.numpy(), Kp.numpy())
 
-    e2e, oneshot_ms = None, None
+    e2e, oneshot_ms, plan_warm = None, None, None
     if world == 1:
         step_host(); barrier()
         t0 = time.perf_counter()
@@ -497,6 +498,10 @@ def main():
         h2d = nao * nao * 8
         d2h = 2 * natm * 3 * 8 if kind == "grad" else 2 * nao * nao * 8
         e2e = {"value": nq / (e2e_ms * 1e-3), "unit": "quartets/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+        if kind != "list":   # a second plan of the same input: the first one of a process also pays for loading the library's code
+            p2 = eri.eri_plan_create(basis, thr, want_grad=(kind == "grad"))
+            s2 = p2.stats(); p2.destroy()
+            plan_warm = {"plan_ms": s2["plan_ms"], "parts": {k: s2["plan_ms_" + k] for k in ("init", "schwarz", "pairs", "units")}}
         if kind != "list":   # the one-shot call of the north star: plan + build + destroy
             barrier(); t0 = time.perf_counter()
             if kind == "grad":
@@ -538,7 +543,7 @@ def main():
             "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": desc, "nao": nao, "nshell": basis.nshell, "quartets_kept": nq, "quartets_total": st["quartets_total"],
                        "pairs_kept": st["pairs_kept"], "canonical_flops": flops, "plan_ms": st["plan_ms"],
-                       "plan_ms_parts": {k: st["plan_ms_" + k] for k in ("init", "schwarz", "pairs", "units")}, "oneshot_ms": oneshot_ms,
+                       "plan_ms_parts": {k: st["plan_ms_" + k] for k in ("init", "schwarz", "pairs", "units")}, "plan_ms_second_plan": plan_warm, "oneshot_ms": oneshot_ms,
                        "l2": "flushed between timed steps (256 MB fill)", "kernel_mode": args.kernel_mode,
                        "parallelism": f"replicated plan, thread blocks dealt round-robin over {world} ranks, NCCL all-reduce of J,K" if world > 1 else "single GPU"},
             "jk_build_ms_per_call": ms, "canonical_tflops": flops / (ms * 1e-3) / 1e12, "fp64_peak_measured_tflops": fp64_peak,
