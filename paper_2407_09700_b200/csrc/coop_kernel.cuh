@@ -351,13 +351,16 @@ __global__ void __launch_bounds__(32 * (CoopTraits<LA, LB, LC, LD, TW, NCH>::WAR
     for (int ps = 0; ps < PASSES; ++ps) {
       const bool own = lane + T * ps < NAB;
       const long ra = (long)(a0 + ia[ps]) * n, rb = (long)(b0 + ib[ps]) * n;
-      const double Dab = own ? f * D[ra + b0 + ib[ps]] : 0.0;
+      // D is symmetric (eri.h): the blocks are read through their transposes, D_ca, D_cb, D_da, D_db, so that the lanes of one
+      // load instruction -- fixed c or d, bra components a or b across the lanes -- touch one row of D instead of NA or NB rows
+      const int ca = a0 + ia[ps], cb = b0 + ib[ps];
+      const double Dab = own ? f * D[rb + ca] : 0.0;
       const double fo = own ? f : 0.0;
       double Dac[NC], Dbc[NC], Dad[ND], Dbd[ND];
 #pragma unroll
-      for (int c = 0; c < NC; ++c) { Dac[c] = D[ra + c0 + c]; Dbc[c] = D[rb + c0 + c]; }
+      for (int c = 0; c < NC; ++c) { const long rc = (long)(c0 + c) * n; Dac[c] = D[rc + ca]; Dbc[c] = D[rc + cb]; }
 #pragma unroll
-      for (int d = 0; d < ND; ++d) { Dad[d] = D[ra + d0 + d]; Dbd[d] = D[rb + d0 + d]; }
+      for (int d = 0; d < ND; ++d) { const long rd = (long)(d0 + d) * n; Dad[d] = D[rd + ca]; Dbd[d] = D[rd + cb]; }
       double jab = 0.0, kac[NC], kbc[NC], kad[ND], kbd[ND];
 #pragma unroll
       for (int c = 0; c < NC; ++c) kac[c] = kbc[c] = 0.0;
