@@ -17,7 +17,8 @@
  *   - atomic orbitals are real solid harmonics, unit-normalised on the sphere, m = -l..+l for every l; shells appear
  *     in input order, `ao_off` is the index of the shell's m = -l function and must equal the running sum of (2l+1);
  *   - matrices are nao x nao, row-major, FP64; units Bohr and Hartree;
- *   - D is assumed symmetric by the J/K build and the gradient (the eight-fold list uses it).
+ *   - D is assumed symmetric by the J/K build, the list digest and the gradient (the eight-fold list uses it, PAPER.md:68;
+ *     the cooperative kernels also read density blocks through their transposes).
  *
  * Memory: every pointer says HOST or DEVICE.  The caller owns every buffer it passes; the library copies what it
  * needs and owns the plan and its workspaces.  Outputs are overwritten, not accumulated.  Device work is enqueued on

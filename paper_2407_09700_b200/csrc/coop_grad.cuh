@@ -155,13 +155,15 @@ __global__ void __launch_bounds__(32 * WARPS, (CoopGradTraits<LA, LB, LC, LD, WA
       const int ia = ab / NB, ib = ab - ia * NB;
       int ax, ay, az, bx, by, bz;
       cart_powers(LA, ia, ax, ay, az); cart_powers(LB, ib, bx, by, bz);
-      const long ra = (long)(a0 + ia) * n, rb = (long)(b0 + ib) * n;
-      const double dab = own ? D[ra + b0 + ib] : 0.0;
+      // D is symmetric: the blocks are read through their transposes (one row of D per load instruction instead of NA or NB rows,
+      // coop_kernel.cuh phase 3)
+      const int ca = a0 + ia, cb = b0 + ib;
+      const double dab = own ? D[(long)cb * n + ca] : 0.0;
       double Dac[NC], Dbc[NC], Dad[ND], Dbd[ND];
 #pragma unroll
-      for (int c = 0; c < NC; ++c) { Dac[c] = own ? D[ra + c0 + c] : 0.0; Dbc[c] = own ? D[rb + c0 + c] : 0.0; }
+      for (int c = 0; c < NC; ++c) { const long rc = (long)(c0 + c) * n; Dac[c] = own ? D[rc + ca] : 0.0; Dbc[c] = own ? D[rc + cb] : 0.0; }
 #pragma unroll
-      for (int d = 0; d < ND; ++d) { Dad[d] = D[ra + d0 + d]; Dbd[d] = D[rb + d0 + d]; }
+      for (int d = 0; d < ND; ++d) { const long rd = (long)(d0 + d) * n; Dad[d] = D[rd + ca]; Dbd[d] = D[rd + cb]; }
       const int ox = (ax * SI + bx * SJ), oy = (ay * SI + by * SJ) + N * G2, oz = (az * SI + bz * SJ) + 2 * N * G2;
       const double fax = (double)ax, fay = (double)ay, faz = (double)az, fbx = (double)bx, fby = (double)by, fbz = (double)bz;
 #pragma unroll 1
