@@ -192,7 +192,7 @@ struct TileTraits {
   static constexpr int NKEEP = NCD + NAT * ND;              // per-thread sums kept over the rows: J_cd, K_ad
   static constexpr int STAGE = max3(reduce_stage_size(NABT), reduce_stage_size(NAT * NC), reduce_stage_size(NB * NC));   // doubles per warp
   static constexpr int RT = rys2_size(N);                    // the class's Rys table, first in the block's shared memory (16-byte aligned)
-  static constexpr size_t SMEM = sizeof(double) * (RT + NW * STAGE + NKEEP * NT);
+  static constexpr size_t SMEM = sizeof(double) * (RT + NW * STAGE + 2 * NKEEP * NT);   // + D_cd, D_ad of every thread, fixed for the block
 };
 
 template <int LA, int LB, int LC, int LD, int TQ, int BI>
@@ -212,6 +212,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
   rys_stage_table<N>(smem, w.rys, tid, NT);
   double* stage = smem + Tr::RT + wy * Tr::STAGE;
   double* keep = smem + Tr::RT + Tr::NW * Tr::STAGE + tid;   // keep[e * NT]: [0, NCD) J_cd ; [NCD, NCD + NAT*ND) K_ad
+  const double* hold = keep + NKEEP * NT;                    // hold[e * NT]: [0, NCD) D_cd ; [NCD, NCD + NAT*ND) D_ad (filled below)
 #pragma unroll
   for (int e = 0; e < NKEEP; ++e) keep[e * NT] = 0.0;
   __syncthreads();
@@ -228,6 +229,21 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
   const int n = w.nao;
   const double* __restrict__ D = w.D;
   double* __restrict__ Jm = w.J; double* __restrict__ Km = w.K;
+  // The density blocks D_cd and D_ad of this thread do not change from row to row (its ket pair is fixed, and the rows of a bra
+  // half share shell a): read once per block.  Per row they were NCD + NAT ND loads whose 32 lanes hit 20-30 different cache
+  // lines each -- a third of the global tag requests of the (ps|ss) kernel (profiles/r02_cfg3.md section 6).
+  {
+    double* hw = keep + NKEEP * NT;
+    const int a0b = bp.ao[i_first].x + t * NAT;
+#pragma unroll
+    for (int c = 0; c < NC; ++c)
+#pragma unroll
+      for (int d = 0; d < ND; ++d) hw[(c * ND + d) * NT] = D[(long)(c0 + c) * n + d0 + d];
+#pragma unroll
+    for (int a = 0; a < NAT; ++a)
+#pragma unroll
+      for (int d = 0; d < ND; ++d) hw[(NCD + a * ND + d) * NT] = D[(long)(a0b + a) * n + d0 + d];
+  }
   int a0 = -1;                         // first Cartesian AO of shell a owned by this thread
   const double thr = w.thr_dev ? *w.thr_dev : w.thr;   // density-weighted call: tau / P_{ab|cd} of this unit (Eq. 8-9)
 
@@ -300,7 +316,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
 #pragma unroll
       for (int c = 0; c < NC; ++c)
 #pragma unroll
-        for (int d = 0; d < ND; ++d) Dcd[c * ND + d] = D[(long)(c0 + c) * n + d0 + d];
+        for (int d = 0; d < ND; ++d) Dcd[c * ND + d] = hold[(c * ND + d) * NT];
       double v[NABT];
 #pragma unroll
       for (int ab = 0; ab < NABT; ++ab) {
@@ -368,7 +384,7 @@ __global__ void __launch_bounds__(32 * BI * TQ, (TileTraits<LA, LB, LC, LD, TQ, 
 #pragma unroll
       for (int a = 0; a < NAT; ++a)
 #pragma unroll
-        for (int d = 0; d < ND; ++d) Dad[a * ND + d] = D[(long)(a0 + a) * n + d0 + d];
+        for (int d = 0; d < ND; ++d) Dad[a * ND + d] = hold[(NCD + a * ND + d) * NT];
       double v[NB * NC];
 #pragma unroll
       for (int b = 0; b < NB; ++b)
