@@ -179,6 +179,13 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
   for (int c = 0; c < NC; ++c)
 #pragma unroll
     for (int d = 0; d < ND; ++d) Dcd_s[32 * (c * ND + d)] = D[(long)(c0 + c) * n + d0 + d];
+  {  // D_ad of this lane is the same for every row of the block (the rows of a bra half share shell a): once, not per row
+    const int a0b = bp.ao[i_first].x;
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+      for (int d = 0; d < ND; ++d) Dad_s[32 * (a * ND + d)] = D[(long)(a0b + a) * n + d0 + d];
+  }
   double keepD[6];   // centre D: -(A + B + C), J then K, summed over the rows of this warp
 #pragma unroll
   for (int e = 0; e < 6; ++e) keepD[e] = 0.0;
@@ -199,10 +206,6 @@ __global__ void __launch_bounds__(32 * BI) tile_grad_kernel(Work w) {
     for (int e = x; e < NA * NB; e += 32) Dab_s[e] = D[(long)(a0 + e / NB) * n + b0 + e % NB];
     for (int e = x & 15; e < NA * NC; e += 16) Dac_s[e] = D[(long)(a0 + e / NC) * n + c0 + e % NC];   // each half stages its own c
     for (int e = x & 15; e < NB * NC; e += 16) Dbc_s[e] = D[(long)(b0 + e / NC) * n + c0 + e % NC];
-#pragma unroll
-    for (int a = 0; a < NA; ++a)
-#pragma unroll
-      for (int d = 0; d < ND; ++d) Dad_s[32 * (a * ND + d)] = D[(long)(a0 + a) * n + d0 + d];
 #pragma unroll
     for (int b = 0; b < NB; ++b)
 #pragma unroll
@@ -411,6 +414,13 @@ __global__ void __launch_bounds__(96 * BI) tile_grad_team_kernel(Work w) {
 #pragma unroll
       for (int d = 0; d < ND; ++d) Dcd_s[32 * (c * ND + d)] = D[(long)(c0 + c) * n + d0 + d];
   }
+  if (t == 1) {   // D_ad of this lane: the same for every row of the block (the first row's barrier publishes it to the team)
+    const int a0b = bp.ao[i_first].x;
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+      for (int d = 0; d < ND; ++d) Dad_s[32 * (a * ND + d)] = D[(long)(a0b + a) * n + d0 + d];
+  }
   double keepD[2] = {0.0, 0.0};   // centre D of this thread's axis: -(A + B + C), J and K, over the rows
   bool any_row = false;
 
@@ -429,12 +439,7 @@ __global__ void __launch_bounds__(96 * BI) tile_grad_team_kernel(Work w) {
       for (int e = x; e < NA * NB; e += 32) Dab_s[e] = D[(long)(a0 + e / NB) * n + b0 + e % NB];
       for (int e = x & 15; e < NA * NC; e += 16) Dac_s[e] = D[(long)(a0 + e / NC) * n + c0 + e % NC];
       for (int e = x & 15; e < NB * NC; e += 16) Dbc_s[e] = D[(long)(b0 + e / NC) * n + c0 + e % NC];
-    } else if (t == 1) {
-#pragma unroll
-      for (int a = 0; a < NA; ++a)
-#pragma unroll
-        for (int d = 0; d < ND; ++d) Dad_s[32 * (a * ND + d)] = D[(long)(a0 + a) * n + d0 + d];
-    } else {
+    } else if (t == 2) {
 #pragma unroll
       for (int b = 0; b < NB; ++b)
 #pragma unroll
