@@ -79,3 +79,19 @@ def test_no_gpu_means_loud_failure(eri):
     h = ctypes.c_void_p()
     rc = eri.lib().eri_plan_create(*args, ctypes.c_double(0.0), 0, None, ctypes.byref(h))
     assert rc == -3   # ERI_ERR_CUDA: no fallback
+
+
+def test_noalloc_entry_point_validates_sizes_without_a_device(eri):
+    """eri_density_group_max_noalloc refuses what its static scratch array cannot hold, before touching the device"""
+    import ctypes
+    L = eri.lib()
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    big = eri.ERI_NOALLOC_MAX_GROUPS + 1
+    rc = L.eri_density_group_max_noalloc(vp(8), ci(4), vp(8), ci(big), vp(8), None)   # (dummy non-null pointers: never dereferenced)
+    assert rc == -1 and b"ERI_NOALLOC_MAX_GROUPS" in L.eri_last_error()
+    assert L.eri_density_group_max_noalloc(vp(8), ci(-1), vp(8), ci(2), vp(8), None) == -1
+    assert L.eri_density_group_max_noalloc(vp(8), ci(4), vp(8), ci(-2), vp(8), None) == -1
+    assert L.eri_density_group_max_noalloc(None, ci(4), vp(8), ci(2), vp(8), None) == -1      # null D
+    assert L.eri_density_group_max_noalloc(vp(8), ci(4), vp(8), ci(2), None, None) == -1      # null P
+    assert L.eri_density_group_max_noalloc(None, ci(0), None, ci(0), None, None) == 0         # nothing to do
+    assert L.eri_plan_dscreen_group_max(None, None, None) == -1
